@@ -1,0 +1,294 @@
+"""Pins of the CPU oracle against what the paper and the physics fix (no GPU, no CUDA path).
+
+Each test names the passage it pins (P:nn = /root/reference/PAPER.md line nn) and the mistake it would catch.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_03857_b200 import workloads
+
+GAMMA = workloads.GAMMA_MGAL
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _golden():
+    rows = []
+    with open(os.path.join(HERE, "golden", "prism_gz_quadrature.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            t = line.split()
+            rows.append((t[0], tuple(map(float, t[1:4])), tuple(map(float, t[4:10])), float(t[10]), float(t[11])))
+    return rows
+
+
+# ---- Eq. 1-3: value, sign, units ------------------------------------------------------------------
+@pytest.mark.parametrize("name,station,box,rho,ref", _golden())
+def test_worked_values_quadrature(name, station, box, rho, ref):
+    """Closed form vs 40-digit quadrature of Newton's law (tests/golden/make_quadrature_pins.py).
+    A dropped term, a wrong sign of any term, atan2 instead of atan, or swapped X/Y roles fails here."""
+    truth = oracle.prism_gz(station, box, rho, GAMMA, prec=1)
+    # long-double closed form: limited by its own cancellation only (case D: far field)
+    lim_ld = 1e-15 if name not in ("D", "Dmirror") else 3e-12
+    assert abs(truth - ref) <= lim_ld * abs(ref)
+    # double closed form: error bounded by eps * gamma*rho * (8 corner terms of size ~ L*ln(L))
+    val = oracle.prism_gz(station, box, rho, GAMMA, prec=0)
+    L = max(abs(b - s) for b, s in zip(box, (station[0],) * 2 + (station[1],) * 2 + (station[2],) * 2))
+    bound = 8 * 2.3e-16 * GAMMA * rho * L * (3 + 2 * math.log(max(L, 2.0)))
+    assert abs(val - ref) <= bound
+
+
+def test_units_bouguer_constant():
+    """Reading C4: 2*pi*gamma*1000 kg/m^3*1 m = 0.041934 mGal (P:60 gamma; BASELINE.json config 1 units)."""
+    assert abs(2 * math.pi * GAMMA * 1000 * 1 - 0.041934) < 5e-7
+
+
+def test_bouguer_slab_limit():
+    """Wide thin slab -> 2*pi*gamma*rho*h (BASELINE.json north_star pin). Wrong sigma parity or a missing
+    Z*atan term destroys this (the slab value is carried almost entirely by the atan terms)."""
+    rho, h = 1000.0, 10.0
+    v = oracle.prism_gz((0, 0, -1), (-1e7, 1e7, -1e7, 1e7, 0, h), rho, GAMMA, prec=1)
+    slab = 2 * math.pi * GAMMA * rho * h
+    assert abs(v - slab) / slab < 1e-6           # finite width: 5.4e-7
+    assert v < slab
+    assert abs(v - 0.41933956087809403485) < 1e-12   # SURVEY.md A.2 slab value (independent quadrature there)
+
+
+def test_point_mass_far_field():
+    """Cube of side a at distance r: gz -> gamma*rho*V*Z/r^3, error O((a/r)^4) (north_star pin)."""
+    a, rho = 100.0, 300.0
+    box = (0, a, 0, a, 1000, 1000 + a)
+    st = (5000.0, 3000.0, -1.0)
+    c = (a / 2, a / 2, 1000 + a / 2)
+    dx, dy, dz = c[0] - st[0], c[1] - st[1], c[2] - st[2]
+    r = math.sqrt(dx * dx + dy * dy + dz * dz)
+    pm = GAMMA * rho * a ** 3 * dz / r ** 3
+    v = oracle.prism_gz(st, box, rho, GAMMA, prec=1)
+    assert abs(v - pm) / pm < 5 * (a / r) ** 4
+    # and the error shrinks like (a/r)^4 when the cube is moved twice as far
+    st2 = (2 * 5000.0 - a / 2, 2 * 3000.0 - a / 2, -2 * (1000 + a / 2 + 1) + 1000 + a / 2)
+    dx, dy, dz = c[0] - st2[0], c[1] - st2[1], c[2] - st2[2]
+    r2 = math.sqrt(dx * dx + dy * dy + dz * dz)
+    v2 = oracle.prism_gz(st2, box, rho, GAMMA, prec=1)
+    pm2 = GAMMA * rho * a ** 3 * dz / r2 ** 3
+    assert abs(v2 - pm2) / pm2 < 5 * (a / r2) ** 4
+
+
+def test_mirror_antisymmetry():
+    """Station mirrored through the prism's horizontal mid-plane: gz -> -gz exactly (needs principal atan, C3)."""
+    box = (0, 100, 0, 100, 1000, 1100)
+    for st in [(5000.0, 3000.0, -1.0), (30.0, 40.0, 900.0), (-200.0, 50.0, 0.0)]:
+        mir = (st[0], st[1], 2 * 1050.0 - st[2])
+        a = oracle.prism_gz(st, box, 300.0, GAMMA, prec=1)
+        b = oracle.prism_gz(mir, box, 300.0, GAMMA, prec=1)
+        assert a > 0 and b < 0
+        assert abs(a + b) <= 1e-15 * abs(a) + 1e-13 * abs(a) * (st[0] > 1000)
+
+
+def test_superposition_eight_subprisms():
+    """Prism split into 8 sub-prisms gives the same gz (north_star pin): catches a wrong p/q/r <-> bound map."""
+    rng = np.random.default_rng(1)
+    for _ in range(20):
+        lo = rng.uniform(-300, 300, 3)
+        sz = rng.uniform(10, 400, 3)
+        lo[2] = rng.uniform(0, 300)
+        mid = lo + sz * rng.uniform(0.2, 0.8, 3)
+        hi = lo + sz
+        st = (rng.uniform(-500, 500), rng.uniform(-500, 500), -rng.uniform(0.5, 50))
+        whole = oracle.prism_gz(st, (lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]), 250.0, GAMMA, prec=1)
+        parts = 0.0
+        for xs in ((lo[0], mid[0]), (mid[0], hi[0])):
+            for ys in ((lo[1], mid[1]), (mid[1], hi[1])):
+                for zs in ((lo[2], mid[2]), (mid[2], hi[2])):
+                    parts += oracle.prism_gz(st, (*xs, *ys, *zs), 250.0, GAMMA, prec=1)
+        assert abs(whole - parts) <= 1e-13 * abs(whole)
+
+
+def test_psi_symmetry_and_guards():
+    """Eq. 2 is symmetric under X<->Y; guards of reading C6 give finite values on edges / faces."""
+    assert oracle.psi(3.0, -7.0, 2.0) == pytest.approx(oracle.psi(-7.0, 3.0, 2.0), rel=1e-15)
+    # hand value: X=Y=Z=1: R=sqrt3; psi = atan(1/sqrt3) - 2 ln(sqrt3+1) = pi/6 - 2 ln(1+sqrt3)
+    assert oracle.psi(1, 1, 1) == pytest.approx(math.pi / 6 - 2 * math.log(1 + math.sqrt(3)), rel=1e-15)
+    # Z = 0: only the log terms;  X = 0: X ln(.) dropped even though ln(R+Y) = ln(0) for Y<0, Z=0
+    assert oracle.psi(2.0, 3.0, 0.0) == pytest.approx(-2 * math.log(math.sqrt(13) + 3) - 3 * math.log(math.sqrt(13) + 2))
+    assert math.isfinite(oracle.psi(0.0, -5.0, 0.0))
+    assert oracle.psi(0.0, -5.0, 0.0) == pytest.approx(5.0 * math.log(5.0))
+    assert oracle.psi(0.0, 0.0, 0.0) == 0.0
+    # station on a prism face / inside a prism stays finite (gz inside a cube centre is 0 by symmetry)
+    assert abs(oracle.prism_gz((0, 0, 0), (-1, 1, -1, 1, -1, 1), 1.0, 1.0)) < 1e-15
+    assert math.isfinite(oracle.prism_gz((0, 0, 0), (0, 1, 0, 1, 0, 1), 1.0, 1.0))
+
+
+# ---- operators on config 1 ----------------------------------------------------------------------------------
+def test_cfg1_positivity_and_extreme_data(cfg1):
+    """Every station is above every prism -> all G_ik > 0 (P:47 geometry, z down: C2).
+    Noise-free data of cfg 1 are ONE 200x200x150 m prism: max/min equal golden cases E and F."""
+    G, wl = cfg1["G"], cfg1["wl"]
+    assert G.min() > 0
+    assert G.min() == pytest.approx(1.8e-8, rel=0.1)
+    g = {r[0]: r[4] for r in _golden()}
+    assert cfg1["d_clean"].max() == pytest.approx(g["E"], rel=1e-12)
+    assert cfg1["d_clean"].min() == pytest.approx(g["F"], rel=1e-11)
+
+
+def test_forward_adjoint_match_tabulated_and_numpy(cfg1):
+    """Eq. 5 and its transpose: matrix-free loops == tabulated G applied by numpy (library routine).
+    A transposed operand or wrong cell<->index map in either loop fails."""
+    wl, mesh, G = cfg1["wl"], cfg1["mesh"], cfg1["G"]
+    u, v, _ = wl.test_vectors()
+    d = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
+    assert np.abs(d - G @ u).max() <= 1e-13 * np.abs(d).max()
+    g = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)
+    assert np.abs(g - G.T @ v).max() <= 1e-13 * np.abs(g).max()
+    cells = np.array([0, 7, 1000, wl.M - 1])
+    gs = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=cells)
+    assert np.allclose(gs, g[cells], rtol=0, atol=1e-18)
+    assert np.abs(oracle.dense_matvec(G, u) - G @ u).max() <= 1e-13 * np.abs(d).max()
+    assert np.abs(oracle.dense_rmatvec(G, v) - G.T @ v).max() <= 1e-13 * np.abs(g).max()
+
+
+def test_dot_product_test(cfg1):
+    """<G u, v> = <u, G^T v> for random u, v."""
+    wl, mesh = cfg1["wl"], cfg1["mesh"]
+    u, v, _ = wl.test_vectors()
+    d = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
+    g = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)
+    a, b = float(d @ v), float(u @ g)
+    assert abs(a - b) <= 1e-12 * max(abs(a), abs(b), np.linalg.norm(d) * np.linalg.norm(v) * 1e-3)
+
+
+def test_whole_mesh_row_sum(cfg1):
+    """forward(u = 1) at station i = gz of the mesh bounding box as ONE prism (superposition over all M cells):
+    exercises every (station, cell) pair and the cell ordering with 8N single-prism evaluations."""
+    wl, mesh = cfg1["wl"], cfg1["mesh"]
+    d = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, np.ones(wl.M))
+    box = (wl.xn[0], wl.xn[-1], wl.yn[0], wl.yn[-1], wl.zn[0], wl.zn[-1])
+    one = np.array([oracle.prism_gz((wl.xo[i], wl.yo[i], wl.zo[i]), box, 1.0, wl.gamma, prec=1) for i in range(wl.N)])
+    assert np.abs(d - one).max() <= 1e-12 * np.abs(one).max()
+    # a box-aligned body is one prism as well: cfg 1's block (reading C13)
+    body = np.array([oracle.prism_gz((wl.xo[i], wl.yo[i], wl.zo[i]), (300, 500, 300, 500, 100, 250), 500.0, wl.gamma,
+                                     prec=1) for i in range(wl.N)])
+    assert np.abs(cfg1["d_clean"] - body).max() <= 1e-12 * np.abs(body).max()
+
+
+def test_grid_symmetries(cfg1):
+    """Centred block under a centred station grid: data symmetric under x-mirror, y-mirror and x<->y."""
+    wl = cfg1["wl"]
+    D = cfg1["d_clean"].reshape(wl.nx, wl.ny)
+    s = np.abs(D).max()
+    assert np.abs(D - D[::-1, :]).max() <= 1e-12 * s
+    assert np.abs(D - D[:, ::-1]).max() <= 1e-12 * s
+    assert np.abs(D - D.T).max() <= 1e-12 * s
+
+
+def test_irregular_mesh_row_sum_and_truth():
+    """Non-cubic, stretched mesh + irregular stations over topography: row sums == one prism; double vs long double."""
+    wl = workloads.make_custom(5, 7, 4, 30.0, 23, seed=3, topo_amp=40.0)
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    d = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, np.ones(wl.M))
+    box = (wl.xn[0], wl.xn[-1], wl.yn[0], wl.yn[-1], wl.zn[0], wl.zn[-1])
+    one = np.array([oracle.prism_gz((wl.xo[i], wl.yo[i], wl.zo[i]), box, 1.0, wl.gamma, prec=1) for i in range(wl.N)])
+    assert np.abs(d - one).max() <= 1e-12 * np.abs(one).max()
+    dt = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, wl.m_true, prec=1)
+    dd = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, wl.m_true, prec=0)
+    assert np.abs(dt - dd).max() <= 1e-12 * np.abs(dt).max()
+
+
+# ---- depth weights (north_star) -----------------------------------------------------------------------
+def test_depth_weights():
+    wl = workloads.make(1)
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    assert np.all(oracle.depth_weights(mesh, 0.0, 25.0) == 1.0)
+    w = oracle.depth_weights(mesh, 2.0, 25.0).reshape(wl.nx, wl.ny, wl.nz)
+    zc = (np.arange(wl.nz) + 0.5) * wl.h
+    assert np.allclose(w[3, 5, :], 1.0 / (zc + 25.0), rtol=1e-15)          # beta=2 -> 1/(z+z0)
+    assert np.all(w == w[0:1, 0:1, :])                                      # depends on the layer only
+    w3 = oracle.depth_weights(mesh, 3.0, 10.0).reshape(wl.nx, wl.ny, wl.nz)
+    assert np.allclose(w3[0, 0, :], (zc + 10.0) ** -1.5, rtol=1e-14)
+    # depth is measured from the mesh top, not from z = 0
+    mesh2 = oracle.Mesh(wl.xn, wl.yn, wl.zn + 500.0)
+    assert np.allclose(oracle.depth_weights(mesh2, 2.0, 25.0), w.ravel(), rtol=1e-15)
+
+
+# ---- data-space system ---------------------------------------------------------------------------
+def test_conditioning_facts(cfg1):
+    """cfg 1 trace/N = 4.946e-3, lambda = 4.946e-5, eig(A) in [7.9e-4, 0.3366], cond = 401."""
+    G, w, lam, wl = cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["wl"]
+    assert cfg1["diag"].sum() / wl.N == pytest.approx(4.946e-3, rel=2e-4)
+    assert lam == pytest.approx(4.946e-5, rel=2e-4)
+    A0 = (G / w ** 2) @ G.T
+    assert np.allclose(cfg1["diag"], np.diag(A0), rtol=1e-12)
+    A = oracle.form_A(G, w, lam)
+    assert np.abs(A - (A0 + lam * np.eye(wl.N))).max() <= 1e-14 * np.abs(A).max()
+    ev = np.linalg.eigvalsh(A0)
+    assert ev[-1] == pytest.approx(0.3366, rel=1e-3)
+    assert (ev[-1] + lam) / (ev[0] + lam) == pytest.approx(401, rel=0.02)
+
+
+def test_cholesky_against_library(cfg1):
+    A = oracle.form_A(cfg1["G"], cfg1["w"], cfg1["lam"])
+    x = oracle.cholesky_solve(A, cfg1["d_obs"])
+    xr = np.linalg.solve(A, cfg1["d_obs"])
+    assert np.abs(x - xr).max() <= 1e-11 * np.abs(xr).max()
+    with pytest.raises(np.linalg.LinAlgError):
+        oracle.cholesky_solve(-np.eye(3), np.ones(3))
+
+
+def test_push_through_identity(cfg1):
+    """Eq. 9: the data-space solution equals the model-space Tikhonov solution
+    (G^T G + lambda W^2)^-1 G^T d  (Eq. 8 with W_d = lambda I, W_m^-1 = W^2).  SURVEY.md A.4: 1.2e-11."""
+    G, w, lam, d = cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    alpha, m_ds = oracle.dataspace_direct(G, w, lam, d)
+    m_ms = oracle.modelspace_direct(G, w, lam, d)
+    assert np.abs(m_ds - m_ms).max() <= 1e-9 * np.abs(m_ms).max()
+    # recovered model: smooth positive body of the right order (A.4 reports [-21.6, 159.2] for its noise draw)
+    assert -40 < m_ds.min() < -5 and 120 < m_ds.max() < 200
+    # a wrong weighting power (W^-1 or W^-4 instead of W^-2) breaks the identity at the 1e-1 level
+    _, m_bad = oracle.dataspace_direct(G, np.sqrt(w), lam, d)
+    assert np.abs(m_bad - m_ms).max() > 1e-2 * np.abs(m_ms).max()
+
+
+def test_cg_vs_direct(cfg1):
+    """CG (C8) converges to the Cholesky solution: k=50 ~2.5e-9, k=100 ~1e-14."""
+    G, w, lam, d = cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    alpha, m = oracle.dataspace_direct(G, w, lam, d)
+    st50, hist50, _ = oracle.cg(w, lam, d, 50, G=G)
+    st100, hist100, _ = oracle.cg(w, lam, d, 100, G=G)
+    s = np.abs(alpha).max()
+    assert np.abs(st50.x - alpha).max() <= 1e-7 * s
+    assert np.abs(st100.x - alpha).max() <= 1e-12 * s
+    assert hist50[0] == pytest.approx(np.linalg.norm(d), rel=1e-14)
+    assert hist50[50] / hist50[0] < 1e-8 and hist100[100] / hist100[0] < 1e-18
+    assert np.abs(oracle.recover_model(G, w, st100.x) - m).max() <= 1e-11 * np.abs(m).max()
+    # recursive residual equals the true residual d - A x
+    A = oracle.form_A(G, w, lam)
+    assert np.abs((d - A @ st50.x) - st50.r).max() <= 1e-12 * np.abs(d).max()
+
+
+def test_cg_first_step_closed_form(cfg1):
+    """One CG step from x0=0 has the closed form x1 = (r.r / r.Ar) r (textbook steepest descent step)."""
+    G, w, lam, d = cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    A = oracle.form_A(G, w, lam)
+    st, hist, ab = oracle.cg(w, lam, d, 1, G=G)
+    a = (d @ d) / (d @ (A @ d))
+    assert ab[0, 0] == pytest.approx(a, rel=1e-13)
+    assert np.allclose(st.x, a * d, rtol=1e-13, atol=0)
+    r1 = d - a * (A @ d)
+    assert np.abs(st.r - r1).max() <= 1e-13 * np.abs(d).max()
+    assert ab[0, 1] == pytest.approx((r1 @ r1) / (d @ d), rel=1e-10)
+
+
+def test_cg_state_injection_and_matrix_free(cfg1):
+    """Resuming from an injected state reproduces the uninterrupted run; matrix-free CG == stored-G CG early on."""
+    wl, mesh, G, w, lam, d = cfg1["wl"], cfg1["mesh"], cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    st10, _, _ = oracle.cg(w, lam, d, 10, G=G)
+    st11, _, _ = oracle.cg(w, lam, d, 11, G=G)
+    st11b, _, _ = oracle.cg(w, lam, d, 1, G=G, state=st10)
+    assert np.array_equal(st11.x, st11b.x) and np.array_equal(st11.p, st11b.p) and st11.rho == st11b.rho
+    stm, _, _ = oracle.cg(w, lam, d, 3, mesh=mesh, obs=(wl.xo, wl.yo, wl.zo), gamma=wl.gamma)
+    st3, _, _ = oracle.cg(w, lam, d, 3, G=G)
+    assert np.abs(stm.x - st3.x).max() <= 1e-11 * np.abs(st3.x).max()
