@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the matrix-free prism-gravity hot path on B200.
+
+A "step" is ONE data-space CG iteration on a BASELINE.json configuration (default: config 5, the largest,
+3.33 M prisms x 178,797 stations): adjoint product G^T p (+ depth weighting W^-2 and the node<->prism
+regrouping), forward product G(.), and the fused CG vector updates -- every row of SURVEY.md 8(a) that runs per
+iteration.  metric = prism-observation pair evaluations per second (2*N*M pairs per step), FP64.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "prism-obs pair evals/s (matrix-free G*m, G^T*v, FP64)"
+UNIT = "pair evals/s"
+
+# FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
+# capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
+FP64_INST_PER_EVAL = {"forward_nodes": 116.0, "adjoint_nodes": 116.0}
+FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 8:
+                continue
+            try:
+                sm.append(float(t[0])); mx.append(float(t[1])); pw.append(float(t[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, t[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            # "under load": samples whose power is within 25% of the max seen
+            pmax = max(pw)
+            load = [s for s, p in zip(sm, pw) if p >= 0.75 * pmax] or sm
+            out.update(sm_mhz=statistics.median(load), sm_max_mhz=max(mx), power_w_max=pmax, samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def cpu_oracle_rate(wl, seconds, sample_note=True):
+    """Times the oracle (as it stands) on a bounded sample of the workload: forward on S stations x all prisms."""
+    import oracle
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    cores = oracle.hardware_threads()
+    rng = np.random.default_rng(7)
+    u = wl.m_true
+
+    def run(S):
+        idx = rng.choice(wl.N, size=min(S, wl.N), replace=False)
+        t0 = time.perf_counter()
+        oracle.forward(mesh, wl.xo[idx], wl.yo[idx], wl.zo[idx], wl.gamma, u, nthreads=cores)
+        return time.perf_counter() - t0, idx.size
+
+    S0 = max(cores, 1)
+    t, s = run(S0)
+    rate = s * wl.M / t
+    S = int(max(S0, min(wl.N, seconds * rate / wl.M)))
+    S = max(cores, (S // cores) * cores)
+    t, s = run(S)
+    return dict(value=s * wl.M / t, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"oracle.forward on {s} seeded stations x all {wl.M} prisms ({s * wl.M:.3g} pairs, {t:.1f} s)")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores.  One step = forward + adjoint restricted
+    to a bounded sample of S stations (2*S*M pairs)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2602_03857_b200 import workloads
+    wl = workloads.make(args.config)
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    cores = oracle.hardware_threads()
+    S = max(1, min(wl.N, int(round(1.0e8 / (2 * wl.M)))))      # ~1e8 pairs per step: seconds on a multicore host
+    S = max(S, min(cores, wl.N))
+    rng = np.random.default_rng(7)
+    idx = rng.choice(wl.N, size=S, replace=False)
+    xo, yo, zo = wl.xo[idx], wl.yo[idx], wl.zo[idx]
+    w = oracle.depth_weights(mesh, wl.beta, wl.z0)
+    p = rng.standard_normal(S)
+
+    def step():
+        g = oracle.adjoint(mesh, xo, yo, zo, wl.gamma, p, nthreads=cores)
+        g /= w * w
+        return oracle.forward(mesh, xo, yo, zo, wl.gamma, g, nthreads=cores)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    pairs = 2.0 * S * wl.M * args.steps
+    val = pairs / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "prisms": wl.M, "stations": wl.N,
+                       "sample": f"{S} seeded stations x all prisms per step (adjoint + forward)"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{S} stations x {wl.M} prisms, adjoint+forward per step"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2602_03857_b200 import binding, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        from paper_2602_03857_b200 import dist as gdist
+        return gdist.bench_sharded(args, METRIC, UNIT)
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    wl = workloads.make(args.config)
+    N, M, Nn = wl.N, wl.M, wl.n_nodes
+    ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+    to = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+
+    # ---- inputs resident in HBM: d_obs = G m_true + noise (GPU forward, parity-checked in tests/), weights, lambda
+    w = ctx.depth_weights(wl.beta, wl.z0)
+    d_clean = ctx.forward(to(wl.m_true))
+    sigma = wl.noise_frac * float(d_clean.abs().max().item())
+    d_obs = d_clean + sigma * to(wl.noise())
+    # lambda = 1e-2 * trace / N, trace/N estimated as the mean Gram diagonal over <= 512 seeded stations
+    nsub = min(N, 512)
+    idx = np.sort(np.random.default_rng(3).choice(N, size=nsub, replace=False))
+    sub = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo[idx], wl.yo[idx], wl.zo[idx], wl.gamma, device=local)
+    lam = wl.lam_factor * float(sub.gram_diag(w).mean().item())
+    sub.close()
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    state = binding.CGState(N, dev)
+
+    def one_step(first):
+        state.resume = not first
+        ctx.dataspace_cg(d_obs, w, lam, 1, state=state, want_m=False)
+
+    # ---- warm-up, then K timed steps (L2 flushed between steps, CUDA events on the launching stream)
+    for k in range(args.warmup):
+        one_step(k == 0)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    launches0 = ctx.launches
+    times = []
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)
+        e0, e1 = ev(), ev()
+        torch.cuda.synchronize()
+        e0.record()
+        one_step(args.warmup == 0 and k == 0)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+    launches = ctx.launches - launches0
+    total_ms = sum(times)
+    pairs_per_step = 2.0 * N * M
+    value = pairs_per_step * args.steps / (total_ms * 1e-3)
+
+    # ---- the two dominant kernels timed alone (same launch configuration), for the roofline object
+    u_vec = to(wl.m_true)
+    dn, gm = torch.empty(N, dtype=torch.float64, device=dev), torch.empty(M, dtype=torch.float64, device=dev)
+
+    def timed(fn, reps):
+        fn()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            e0, e1 = ev(), ev()
+            torch.cuda.synchronize()
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return statistics.median(ts)
+
+    reps = max(1, min(3, args.steps))
+    t_fwd = timed(lambda: ctx.forward(u_vec, out=dn), reps)
+    t_adj = timed(lambda: ctx.adjoint(d_obs, out=gm), reps)
+    clocks = sampler.stop()
+
+    evals = float(N) * Nn
+    dom, t_dom = ("forward_nodes", t_fwd) if t_fwd >= t_adj else ("adjoint_nodes", t_adj)
+    inst = FP64_INST_PER_EVAL[dom] * evals
+    achieved = inst / (t_dom * 1e-3) / 1e12
+    peak_nominal = 148 * FP64_LANES_PER_SM * 1.965e9 / 1e12
+    probe_rate, _ = binding.fp64_peak_probe(local, 100000)
+    clk = clocks.get("sm_mhz") or 1965.0
+    roofline = {
+        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_nominal,
+        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": None,
+        "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz (nominal, DESIGN.md); DFMA probe in this run: "
+                       f"{probe_rate / 1e12:.2f} T inst/s",
+        "frac_of_probe": achieved / (probe_rate / 1e12),
+        "frac_at_held_clock": achieved / (148 * FP64_LANES_PER_SM * clk * 1e6 / 1e12),
+        "fp64_inst_per_eval": FP64_INST_PER_EVAL[dom], "evals_per_launch": evals,
+        "ms_forward": t_fwd, "ms_adjoint": t_adj,
+        "pairs_per_s_forward": N * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": N * M / (t_adj * 1e-3),
+    }
+
+    # ---- end to end through the host-buffer C-ABI call: H2D d_obs, weights, 1 CG iteration + model recovery,
+    #      D2H alpha and m, every step
+    e2e = None
+    if not args.no_e2e:
+        dh = d_obs.cpu().pin_memory()
+        ah = torch.empty(N, dtype=torch.float64).pin_memory()
+        mh = torch.empty(M, dtype=torch.float64).pin_memory()
+        ctx.dataspace_cg_host(dh, wl.beta, wl.z0, lam, 1, ah, mh)      # warm
+        nrep = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(nrep):
+            ctx.dataspace_cg_host(dh, wl.beta, wl.z0, lam, 1, ah, mh)
+        dt = time.perf_counter() - t0
+        e2e = {"value": 3.0 * N * M * nrep / dt, "unit": UNIT, "h2d_bytes_per_step": 8 * N,
+               "d2h_bytes_per_step": 8 * (N + M), "ms_per_step": 1e3 * dt / nrep,
+               "call": "grav_dataspace_cg_host(iters=1): H2D d_obs, depth weights, 1 CG iteration (adjoint+forward) "
+                       "+ model recovery (adjoint) = 3*N*M pairs, D2H alpha+m"}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu = cpu_oracle_rate(wl, args.cpu_seconds)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "s_per_cg_iter": total_ms / args.steps * 1e-3,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "prisms": M, "stations": N, "nodes": Nn, "pairs_per_step": pairs_per_step,
+                   "step": "one data-space CG iteration (G^T p, W^-2, G(.), fused vector ops)",
+                   "l2": "flushed between steps (256 MiB write)", "lambda": lam,
+                   "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    ctx.close()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,146 @@
+/* grav.h -- C ABI of libgrav.so: matrix-free FP64 prism-gravity operator and data-space CG on one B200 (sm_100a).
+ *
+ * What is computed (citations: P:nn = PAPER.md line nn of arxiv/paper_2602_03857; BJ = BASELINE.json north_star):
+ *   G_ik = gamma * sum_{p,q,r in {1,2}} (-1)^(p+q+r) Psi(x_p - xo_i, y_q - yo_i, z_r - zo_i)        P:49-52  Eq. 1
+ *   Psi(X,Y,Z) = Z atan(XY/(ZR)) - X ln(R+Y) - Y ln(R+X),  R = sqrt(X^2+Y^2+Z^2)                     P:54-58  Eq. 2-3
+ *   d = G u                                                                                           P:68-74  Eq. 5-6
+ *   g = G^T v                                                                                         P:98-110 (G^T of Eq. 9-11)
+ *   w_k = (zc_k + z0)^(-beta/2), zc_k = depth of the cell centre below the mesh top                   P:85; BJ
+ *   (G W^-2 G^T + lambda I) alpha = d_obs by CG,  m = W^-2 G^T alpha                                  P:101-118 Eq. 10-11; BJ
+ *
+ * Conventions.  z is positive DOWN.  Cell (i,j,k), 0-based, has flat index (i*ny + j)*nz + k (z fastest) and
+ * bounds [xn[i],xn[i+1]] x [yn[j],yn[j+1]] x [zn[k],zn[k+1]].  Stations are SoA (obs_x, obs_y, obs_z).
+ * gamma = 6.674e-6 gives gz in mGal for densities in kg/m^3 and lengths in m.  All arithmetic is FP64.
+ *
+ * Pointers.  Names ending in _host are HOST pointers (pageable or pinned), names ending in _dev are DEVICE pointers
+ * on the context's device.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *
+ * Ownership.  grav_mesh_create copies the node and station coordinates to the device (its only allocation,
+ * <= 4.4 MB at 178,797 stations; freed by grav_mesh_destroy).  EVERY other device byte belongs to the caller:
+ * inputs, outputs and one workspace block (grav_workspace_bytes / grav_set_workspace) that must stay alive and
+ * must not be touched by the caller while a call that uses it is in flight.
+ *
+ * Execution.  *_dev entry points enqueue kernels on `stream` and return without synchronising (CG scalars stay
+ * on the device).  *_host entry points copy in, compute, copy out and synchronise `stream` before returning.
+ * Results are deterministic (fixed reduction orders, no atomics on data).
+ *
+ * Errors.  Every call returns a grav_status; no exception crosses the ABI; grav_last_error() returns a
+ * thread-local message for the last non-OK status.  There is no CPU fallback anywhere in this library.
+ */
+#ifndef GRAV_H_
+#define GRAV_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct grav_ctx grav_ctx; /* opaque */
+
+typedef enum {
+    GRAV_OK = 0,
+    GRAV_EINVAL = -1,  /* NULL pointer, non-positive size, non-increasing node coordinates, bad mode */
+    GRAV_ENOMEM = -2,  /* host or device allocation of the geometry copy failed */
+    GRAV_ECUDA = -3,   /* a CUDA runtime call or kernel launch failed (message has the CUDA error string) */
+    GRAV_ESTATE = -4,  /* workspace not set / too small, or stored G requested before grav_store_g */
+    GRAV_ENOTFIT = -5  /* stored G does not fit in the workspace given */
+} grav_status;
+
+/* operator modes */
+enum {
+    GRAV_MATRIX_FREE = 0, /* closed form evaluated on the fly for every station x node pair (BJ kernels 1, 2) */
+    GRAV_STORED_F64 = 1,  /* G tabulated once as N x M doubles, products are HBM-bound GEMV (BJ kernel 4) */
+    GRAV_STORED_F32 = 2   /* G stored as float (the paper's precision), accumulated in FP64 */
+};
+
+/* Device-resident CG state for resuming / single-step injection (SURVEY.md 8(c) protocol P1).
+ * x, r, p: N doubles each; rho: 1 double (= r.r).  resume = 0: the solver initialises x=0, r=p=d_obs and
+ * overwrites the state on return; resume != 0: the solver continues from the state given. */
+typedef struct {
+    double* x_dev;
+    double* r_dev;
+    double* p_dev;
+    double* rho_dev;
+    int resume;
+} grav_cg_state;
+
+/* Create a context for a rectilinear nx x ny x nz prism mesh and nobs stations (mesh of prisms
+ * defined by their vertices; stations (x0_i, y0_i[, z0_i])).
+ * xn_host[nx+1], yn_host[ny+1], zn_host[nz+1]: node coordinates, strictly increasing; z down.
+ * obs_*_host[nobs]: station coordinates.  gamma: gravitational constant in the caller's units.
+ * device: CUDA device ordinal.  Errors: GRAV_EINVAL, GRAV_ENOMEM, GRAV_ECUDA. */
+grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const double* xn_host, const double* yn_host,
+                             const double* zn_host, long long nobs, const double* obs_x_host,
+                             const double* obs_y_host, const double* obs_z_host, double gamma, int device);
+void grav_mesh_destroy(grav_ctx* ctx);
+
+/* Problem sizes: out[0]=N stations, out[1]=M prisms, out[2]=number of mesh nodes (nx+1)(ny+1)(nz+1). */
+grav_status grav_sizes(const grav_ctx* ctx, long long out[3]);
+
+/* Bytes of caller-owned device workspace needed for `mode` (GRAV_MATRIX_FREE, or the matrix-free block plus the
+ * N x M stored G in FP64 / FP32).  0 on error. */
+size_t grav_workspace_bytes(const grav_ctx* ctx, int mode);
+/* Hand the workspace to the context (256-byte aligned).  Invalidates a previously stored G.
+ * Errors: GRAV_EINVAL (NULL / misaligned), GRAV_ESTATE (smaller than the matrix-free block). */
+grav_status grav_set_workspace(grav_ctx* ctx, void* ws_dev, size_t bytes);
+
+/* d = G u, matrix-free (Eq. 5-6; BJ kernel 1).  u_dev[M] -> d_dev[N]. */
+grav_status grav_forward(grav_ctx* ctx, const double* u_dev, double* d_dev, void* stream);
+/* g = G^T v, matrix-free (BJ kernel 2).  v_dev[N] -> g_dev[M]. */
+grav_status grav_adjoint(grav_ctx* ctx, const double* v_dev, double* g_dev, void* stream);
+/* w_k = (zc_k + z0)^(-beta/2) (BJ).  w_dev[M].  Requires zc_k + z0 > 0 for every layer (else GRAV_EINVAL). */
+grav_status grav_depth_weights(grav_ctx* ctx, double beta, double z0, double* w_dev, void* stream);
+
+/* Conjugate gradients on (G W^-2 G^T + lambda I) alpha = d_obs (Eq. 10-11 with W_m = W^-2,
+ * W_d = lambda I, m_ref = 0; textbook Hestenes-Stiefel, x0 = 0).  Runs exactly `iters` iterations when rtol = 0;
+ * with rtol > 0 the iteration freezes (remaining launches become no-ops) once ||r||_2 <= rtol * ||d_obs||_2.
+ * mode: operator used for the products (stored modes need grav_store_g first).
+ * state: NULL or see grav_cg_state.   alpha_dev[N]: solution.   m_dev[M] or NULL: m = W^-2 G^T alpha.
+ * hist_dev[iters+1] or NULL: ||r||_2 before the first and after every iteration (recursive residual).
+ * ab_dev[2*iters] or NULL: step scalars a_j (step length), b_j (direction update) of every iteration. */
+grav_status grav_dataspace_cg(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda, int iters,
+                              double rtol, int mode, grav_cg_state* state, double* alpha_dev, double* m_dev,
+                              double* hist_dev, double* ab_dev, void* stream);
+
+/* Tabulate G (N x M row-major, prism index fastest; "global memory (sensitivity matrix)", Listing 1)
+ * into the workspace in FP64 (fp32 = 0) or FP32 (fp32 != 0).  GRAV_ENOTFIT if the workspace is too small. */
+grav_status grav_store_g(grav_ctx* ctx, int fp32, void* stream);
+/* d = G u and g = G^T v with the stored G (HBM-bound GEMV, BJ kernel 4; "matrix multiplications"). */
+grav_status grav_forward_stored(grav_ctx* ctx, const double* u_dev, double* d_dev, void* stream);
+grav_status grav_adjoint_stored(grav_ctx* ctx, const double* v_dev, double* g_dev, void* stream);
+/* Device pointer / element size (8 or 4; 0 if none) of the stored G, for inspection by tests. */
+grav_status grav_stored_g(const grav_ctx* ctx, const void** g_dev, int* elem_bytes);
+
+/* diag_dev[N] = diag(G W^-2 G^T)_ii = sum_k G_ik^2 / w_k^2, matrix-free per-pair evaluation (its sum is the
+ * trace that fixes lambda = 1e-2 * trace / N, BJ config 1). */
+grav_status grav_gram_diag(grav_ctx* ctx, const double* w_dev, double* diag_dev, void* stream);
+
+/* Small problems (N <= 1024, needs a stored FP64 G): form A = G W^-2 G^T + lambda I explicitly and solve
+ * A alpha = d_obs by Cholesky on the device (BJ config 1 "solved both directly and by CG").
+ * A_dev: N*N doubles of caller scratch (holds the factor on return).  m_dev[M] or NULL. */
+grav_status grav_direct_solve(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda,
+                              double* A_dev, double* alpha_dev, double* m_dev, void* stream);
+
+/* End-to-end variants with HOST buffers: host->device copy of the inputs, the same kernels, device->host copy
+ * of the result, then cudaStreamSynchronize(stream).  Staging buffers live in the workspace. */
+grav_status grav_forward_host(grav_ctx* ctx, const double* u_host, double* d_host, void* stream);
+grav_status grav_adjoint_host(grav_ctx* ctx, const double* v_host, double* g_host, void* stream);
+grav_status grav_dataspace_cg_host(grav_ctx* ctx, const double* dobs_host, double beta, double z0, double lambda,
+                                   int iters, double rtol, int mode, double* alpha_host, double* m_host,
+                                   double* hist_host, void* stream);
+
+/* Launch accounting: number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+long long grav_launch_count(const grav_ctx* ctx);
+/* FP64 DFMA-only microbenchmark: runs `iters` dependent-chain-free DFMA per thread on the whole device and
+ * returns the number of FP64 thread-instructions executed in *ninstr and the elapsed ms in *ms (synchronises).
+ * Used to confirm the FP64 pipe peak in the same run as the roofline numbers. */
+grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* ms);
+
+/* Thread-local message of the last failure on this thread ("" if none). */
+const char* grav_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAV_H_ */

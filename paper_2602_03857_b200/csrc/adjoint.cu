@@ -1,0 +1,89 @@
+// adjoint.cu -- matrix-free g = G^T v in node-shared form (BASELINE.json north_star kernel 2).
+//
+//   T_n = sum_i v_i Psi(node_n - obs_i);   g_k = gamma * sum_pqr sigma T[corner_pqr(k)]   (nodeops.cu)
+//
+// Transposed tiling: one thread owns KC consecutive nodes of one node column (their z and accumulators live in
+// registers); stations are staged through shared memory in tiles and read at the same address by every thread
+// (broadcast).  X, Y, X*Y, X^2+Y^2 are computed once per (thread, station) and shared by the KC nodes.
+// Every node is owned by exactly one thread: no atomics.  Station chunks give partial[chunk][Nn], added in
+// fixed order by adjoint_reduce.
+#include "grav_internal.cuh"
+#include "psi.cuh"
+
+namespace grav {
+
+constexpr int kAdjObsTile = 256;
+
+template <int TPB, int KC>
+__global__ void __launch_bounds__(TPB) adjoint_nodes_kernel(Geom g, const double* __restrict__ v,
+                                                             double* __restrict__ partial, int ncg, int obs_per_chunk,
+                                                             const int* __restrict__ done) {
+    if (done && *done) return;
+    __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
+    const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
+    const long long nthreads = (long long)g.ncol * ncg;
+    const bool valid = t < nthreads;
+    const long long tl = valid ? t : nthreads - 1;
+    const int cg = (int)(tl / g.ncol);        // column index fastest: lanes of a warp are neighbouring columns
+    const int col = (int)(tl - (long long)cg * g.ncol);
+    const int a = col / g.nyp, b = col - a * g.nyp;
+    const int c0 = cg * KC;
+    const double xa = g.xn[a], yb = g.yn[b];
+    double zc[KC], acc[KC];
+#pragma unroll
+    for (int k = 0; k < KC; ++k) {
+        zc[k] = g.zn[min(c0 + k, g.nzp - 1)];
+        acc[k] = 0.0;
+    }
+    const long long i0 = (long long)blockIdx.y * obs_per_chunk;
+    const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
+    for (long long base = i0; base < i1; base += kAdjObsTile) {
+        const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
+        __syncthreads();
+        for (int j = threadIdx.x; j < cnt; j += TPB)
+            s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
+        __syncthreads();
+        for (int j = 0; j < cnt; ++j) {
+            const double4 o = s_obs[j];
+            const double X = xa - o.x, Y = yb - o.y;
+            const double XY = X * Y;
+            const double Q = fma(Y, Y, X * X);
+#pragma unroll
+            for (int k = 0; k < KC; ++k) {
+                const double Z = zc[k] - o.z;
+                acc[k] = fma(o.w, GRAV_PSI(X, Y, Z, XY, Q), acc[k]);
+            }
+        }
+    }
+    if (valid) {
+        double* out = partial + (long long)blockIdx.y * g.Nn + (long long)col * g.nzp + c0;
+#pragma unroll
+        for (int k = 0; k < KC; ++k)
+            if (c0 + k < g.nzp) out[k] = acc[k];
+    }
+}
+
+__global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __restrict__ partial,
+                                      double* __restrict__ tnode) {
+    long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= Nn) return;
+    double s = 0.0;
+    for (int ch = 0; ch < nchunk; ++ch) s += partial[(long long)ch * Nn + n];
+    tnode[n] = s;
+}
+
+cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
+    const Plan& p = c->plan;
+    dim3 grid(p.adj_blocks, p.adj_nchunk);
+    adjoint_nodes_kernel<128, 8><<<grid, 128, 0, s>>>(c->g, v, partial, p.adj_ncg, p.adj_obs_per_chunk, done);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s) {
+    adjoint_reduce_kernel<<<(unsigned)((c->g.Nn + 255) / 256), 256, 0, s>>>(c->g.Nn, c->plan.adj_nchunk, partial, tnode);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace grav

@@ -1,0 +1,96 @@
+// forward.cu -- matrix-free d = G u in node-shared form (BASELINE.json north_star kernel 1).
+//
+//   d_i = gamma * sum_n c_n Psi(node_n - obs_i),   c = S^T u  (nodeops.cu)          PAPER.md:49-74, Eq. 1-6
+//
+// Tiling: one thread owns one station (coordinates and accumulator in registers); a block owns a tile of
+// stations and a chunk of node columns; the node coefficients c_n of the chunk are read by every thread at the
+// same address (broadcast).  X, Y, X*Y and X^2+Y^2 are constant down a node column and hoisted out of the
+// z-loop.  Chunk partial sums go to partial[chunk][N]; forward_reduce adds them in fixed order (deterministic).
+#include "grav_internal.cuh"
+#include "psi.cuh"
+
+namespace grav {
+
+template <int TPB>
+__global__ void __launch_bounds__(TPB) forward_nodes_kernel(Geom g, const double* __restrict__ cnode,
+                                                             double* __restrict__ partial, int cols_per_chunk,
+                                                             const int* __restrict__ done) {
+    if (done && *done) return;
+    const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
+    const long long il = i < g.N ? i : g.N - 1;
+    const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
+    const int col0 = blockIdx.y * cols_per_chunk;
+    const int col1 = min(col0 + cols_per_chunk, g.ncol);
+    double acc = 0.0;
+    int a = col0 / g.nyp, b = col0 - a * g.nyp;
+    double X = __ldg(g.xn + a) - xo;
+    for (int col = col0; col < col1; ++col) {
+        const double Y = __ldg(g.yn + b) - yo;
+        const double XY = X * Y;
+        const double Q = fma(Y, Y, X * X);
+        const double* __restrict__ cc = cnode + (long long)col * g.nzp;
+        double colacc = 0.0;
+        for (int c = 0; c < g.nzp; ++c) {
+            const double Z = __ldg(g.zn + c) - zo;
+            const double coef = __ldg(cc + c);
+            colacc = fma(coef, GRAV_PSI(X, Y, Z, XY, Q), colacc);
+        }
+        acc += colacc;
+        if (++b == g.nyp) {
+            b = 0;
+            ++a;
+            if (a < g.nxp) X = __ldg(g.xn + a) - xo;
+        }
+    }
+    if (i < g.N) partial[(long long)blockIdx.y * g.N + i] = acc;
+}
+
+// d = scale * sum_chunks partial (+ lam * p).  With dotp != NULL also writes block partials of p . d (CG: delta).
+__global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N, int nchunk,
+                                                                      const double* __restrict__ partial, double scale,
+                                                                      double lam, const double* __restrict__ p,
+                                                                      double* __restrict__ d, double* __restrict__ dotp,
+                                                                      const int* __restrict__ done) {
+    if (done && *done) return;
+    __shared__ double sh[kDotThreads];
+    double loc = 0.0;
+    for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
+        double s = 0.0;
+        for (int ch = 0; ch < nchunk; ++ch) s += partial[(long long)ch * N + i];
+        double val = scale * s;
+        if (p) {
+            double pi = p[i];
+            val = fma(lam, pi, val);
+            loc = fma(pi, val, loc);
+        }
+        d[i] = val;
+    }
+    if (dotp) {
+        sh[threadIdx.x] = loc;
+        __syncthreads();
+        for (int s = kDotThreads / 2; s > 0; s >>= 1) {
+            if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) dotp[blockIdx.x] = sh[0];
+    }
+}
+
+cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
+    const Plan& p = c->plan;
+    dim3 grid(p.fwd_tiles, p.fwd_nchunk);
+    forward_nodes_kernel<128><<<grid, 128, 0, s>>>(c->g, cnode, partial, p.fwd_cols_per_chunk, done);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double scale, double lam, const double* p,
+                                  double* d, double* dot_partial, const CgScalars* sc, cudaStream_t s) {
+    const int* done = sc ? &sc->done : nullptr;
+    forward_reduce_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, c->plan.fwd_nchunk, partial, scale, lam, p, d,
+                                                             dot_partial, done);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace grav

@@ -1,0 +1,488 @@
+// grav_api.cu -- the C ABI of include/grav.h: context, workspace layout, call sequencing.  No arithmetic of the
+// method lives here except the order in which kernels are enqueued.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "grav_internal.cuh"
+
+using namespace grav;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+grav_status fail(grav_status st, const char* fmt, const char* a = "", const char* b = "") {
+    snprintf(g_err, sizeof(g_err), fmt, a, b);
+    return st;
+}
+grav_status cuda_fail(cudaError_t e, const char* where) {
+    return fail(GRAV_ECUDA, "%s: %s", where, cudaGetErrorString(e));
+}
+#define CK(call, where)                                      \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) return cuda_fail(e__, where); \
+    } while (0)
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// Launch plan: enough blocks to fill 148 SMs several times over, fixed per context => deterministic sums.
+void make_plan(const Geom& g, Plan& p) {
+    const int target_blocks = 148 * 16;
+    // forward: 128 stations per block; split the node columns into chunks when the station tiles are few
+    p.fwd_tpb = 128;
+    p.fwd_obs_per_thread = 1;
+    p.fwd_tiles = ceil_div(g.N, p.fwd_tpb * p.fwd_obs_per_thread);
+    int want = ceil_div(target_blocks, p.fwd_tiles);
+    if (want > g.ncol) want = g.ncol;
+    if (want > 1024) want = 1024;
+    if (want < 1) want = 1;
+    p.fwd_cols_per_chunk = ceil_div(g.ncol, want);
+    p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
+    // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
+    p.adj_tpb = 128;
+    p.adj_kc = 8;
+    p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
+    p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
+    want = ceil_div(target_blocks, p.adj_blocks);
+    int maxchunk = ceil_div(g.N, 64);
+    if (want > maxchunk) want = maxchunk;
+    if (want > 256) want = 256;
+    if (want < 1) want = 1;
+    p.adj_obs_per_chunk = ceil_div(g.N, want);
+    p.adj_nchunk = ceil_div(g.N, p.adj_obs_per_chunk);
+}
+
+void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t D = sizeof(double);
+    L.cnode = take(g.Nn * D);
+    L.tnode = take(g.Nn * D);
+    L.fwd_partial = take((size_t)p.fwd_nchunk * g.N * D);
+    L.adj_partial = take((size_t)p.adj_nchunk * g.Nn * D);
+    L.gcell = take(g.M * D);
+    L.cg_x = take(g.N * D);
+    L.cg_r = take(g.N * D);
+    L.cg_p = take(g.N * D);
+    L.cg_q = take(g.N * D);
+    L.cg_w = take(g.M * D);
+    L.dot_partial = take(2 * kDotBlocks * D);
+    L.scalars = take(sizeof(CgScalars) + 64);
+    L.stage_m = take(g.M * D);
+    L.stage_n = take(g.N * D);
+    L.stage_hist = take(4096 * D);
+    L.matfree_end = off;
+    L.gemvt_partial = take((size_t)gemvt_chunks(g.N) * g.M * D);
+    L.gstore = off;
+}
+
+template <class T> T* wsp(grav_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
+
+grav_status check_ready(grav_ctx* c) {
+    if (!c) return fail(GRAV_EINVAL, "NULL context");
+    if (!c->ws) return fail(GRAV_ESTATE, "workspace not set (grav_set_workspace)");
+    return GRAV_OK;
+}
+
+struct DeviceGuard {
+    int prev;
+    bool ok;
+    explicit DeviceGuard(int dev) : prev(0), ok(true) {
+        if (cudaGetDevice(&prev) != cudaSuccess) ok = false;
+        if (ok && prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { cudaSetDevice(prev); }
+};
+
+// node sums T = sum_i v_i Psi(node - obs_i) into ws.tnode
+grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cudaStream_t s) {
+    double* part = wsp<double>(c, c->lay.adj_partial);
+    double* tn = wsp<double>(c, c->lay.tnode);
+    if (c->plan.adj_nchunk == 1) {
+        CK(launch_adjoint_nodes(c, v, tn, done, s), "adjoint_nodes");
+    } else {
+        CK(launch_adjoint_nodes(c, v, part, done, s), "adjoint_nodes");
+        CK(launch_adjoint_reduce(c, part, tn, s), "adjoint_reduce");
+    }
+    return GRAV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* grav_last_error(void) { return g_err; }
+
+grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const double* xn, const double* yn,
+                             const double* zn, long long nobs, const double* ox, const double* oy, const double* oz,
+                             double gamma, int device) {
+    if (!out) return fail(GRAV_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || nobs <= 0) return fail(GRAV_EINVAL, "nx, ny, nz, nobs must be positive");
+    if (!xn || !yn || !zn || !ox || !oy || !oz) return fail(GRAV_EINVAL, "NULL coordinate array");
+    if (!(gamma == gamma)) return fail(GRAV_EINVAL, "gamma is NaN");
+    if ((long long)(nx + 1) * (ny + 1) > 2000000000LL) return fail(GRAV_EINVAL, "too many node columns");
+    const double* arrs[3] = {xn, yn, zn};
+    const int lens[3] = {nx + 1, ny + 1, nz + 1};
+    for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < lens[a]; ++i) {
+            if (!std::isfinite(arrs[a][i])) return fail(GRAV_EINVAL, "non-finite node coordinate");
+            if (i && !(arrs[a][i] > arrs[a][i - 1])) return fail(GRAV_EINVAL, "node coordinates must be strictly increasing");
+        }
+    for (long long i = 0; i < nobs; ++i)
+        if (!std::isfinite(ox[i]) || !std::isfinite(oy[i]) || !std::isfinite(oz[i]))
+            return fail(GRAV_EINVAL, "non-finite station coordinate");
+    int ndev = 0;
+    CK(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount");
+    if (device < 0 || device >= ndev) return fail(GRAV_EINVAL, "bad device ordinal");
+    DeviceGuard dg(device);
+    if (!dg.ok) return fail(GRAV_ECUDA, "cudaSetDevice failed");
+
+    grav_ctx* c = new (std::nothrow) grav_ctx();
+    if (!c) return fail(GRAV_ENOMEM, "host allocation failed");
+    memset(c, 0, sizeof(*c));
+    Geom& g = c->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.nxp = nx + 1; g.nyp = ny + 1; g.nzp = nz + 1;
+    g.ncol = g.nxp * g.nyp;
+    g.N = nobs;
+    g.M = (long long)nx * ny * nz;
+    g.Nn = (long long)g.ncol * g.nzp;
+    g.gamma = gamma;
+    c->device = device;
+
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + 6 * 32;   // each array 256-byte aligned
+    std::vector<double> host;
+    try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
+    void* dev = nullptr;
+    cudaError_t e = cudaMalloc(&dev, nd * sizeof(double));
+    if (e != cudaSuccess) { delete c; return fail(GRAV_ENOMEM, "cudaMalloc of geometry failed: %s", cudaGetErrorString(e)); }
+    size_t off = 0;
+    auto put = [&](const double* src, size_t n) {
+        const double* d = reinterpret_cast<const double*>(dev) + off;
+        memcpy(host.data() + off, src, n * sizeof(double));
+        off = (off + n + 31) & ~(size_t)31;
+        return d;
+    };
+    g.xn = put(xn, g.nxp); g.yn = put(yn, g.nyp); g.zn = put(zn, g.nzp);
+    g.xo = put(ox, nobs); g.yo = put(oy, nobs); g.zo = put(oz, nobs);
+    e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaMemcpy geometry"); }
+    c->geom_dev = dev;
+    make_plan(g, c->plan);
+    make_layout(g, c->plan, c->lay);
+    *out = c;
+    return GRAV_OK;
+}
+
+void grav_mesh_destroy(grav_ctx* c) {
+    if (!c) return;
+    DeviceGuard dg(c->device);
+    if (c->geom_dev) cudaFree(c->geom_dev);
+    delete c;
+}
+
+grav_status grav_sizes(const grav_ctx* c, long long out[3]) {
+    if (!c || !out) return fail(GRAV_EINVAL, "NULL argument");
+    out[0] = c->g.N; out[1] = c->g.M; out[2] = c->g.Nn;
+    return GRAV_OK;
+}
+
+size_t grav_workspace_bytes(const grav_ctx* c, int mode) {
+    if (!c) return 0;
+    if (mode == GRAV_MATRIX_FREE) return c->lay.matfree_end;
+    if (mode == GRAV_STORED_F64) return c->lay.gstore + align_up((size_t)c->g.N * c->g.M * 8);
+    if (mode == GRAV_STORED_F32) return c->lay.gstore + align_up((size_t)c->g.N * c->g.M * 4);
+    return 0;
+}
+
+grav_status grav_set_workspace(grav_ctx* c, void* ws, size_t bytes) {
+    if (!c || !ws) return fail(GRAV_EINVAL, "NULL argument");
+    if ((uintptr_t)ws & 255) return fail(GRAV_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < c->lay.matfree_end) return fail(GRAV_ESTATE, "workspace smaller than grav_workspace_bytes(GRAV_MATRIX_FREE)");
+    c->ws = (char*)ws;
+    c->ws_bytes = bytes;
+    c->stored_elem = 0;
+    return GRAV_OK;
+}
+
+long long grav_launch_count(const grav_ctx* c) { return c ? c->launches : 0; }
+
+grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!u || !d) return fail(GRAV_EINVAL, "NULL vector");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    double* cn = wsp<double>(c, c->lay.cnode);
+    double* part = wsp<double>(c, c->lay.fwd_partial);
+    CK(launch_cell_to_node(c, u, nullptr, cn, s), "cell_to_node");
+    CK(launch_forward_nodes(c, cn, part, nullptr, s), "forward_nodes");
+    CK(launch_forward_reduce(c, part, c->g.gamma, 0.0, nullptr, d, nullptr, nullptr, s), "forward_reduce");
+    return GRAV_OK;
+}
+
+grav_status grav_adjoint(grav_ctx* c, const double* v, double* gout, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!v || !gout) return fail(GRAV_EINVAL, "NULL vector");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    st = adjoint_to_tnode(c, v, nullptr, s);
+    if (st) return st;
+    CK(launch_node_to_cell(c, wsp<double>(c, c->lay.tnode), nullptr, c->g.gamma, gout, s), "node_to_cell");
+    return GRAV_OK;
+}
+
+grav_status grav_depth_weights(grav_ctx* c, double beta, double z0, double* w, void* stream) {
+    if (!c || !w) return fail(GRAV_EINVAL, "NULL argument");
+    if (!(beta == beta) || !(z0 == z0)) return fail(GRAV_EINVAL, "NaN parameter");
+    DeviceGuard dg(c->device);
+    // zc_k + z0 > 0 for the shallowest layer is enough (zc increases with k).  zn is only on the device;
+    // the first layer's half-thickness is positive, so z0 > -that.  Conservative host-side check: z0 >= 0 or
+    // fetch the two top nodes.
+    if (!(z0 >= 0.0)) {
+        double z01[2];
+        CK(cudaMemcpy(z01, c->g.zn, 2 * sizeof(double), cudaMemcpyDeviceToHost), "cudaMemcpy zn");
+        if (!(0.5 * (z01[1] - z01[0]) + z0 > 0.0)) return fail(GRAV_EINVAL, "zc + z0 must be positive");
+    }
+    CK(launch_depth_weights(c, beta, z0, w, (cudaStream_t)stream), "depth_weights");
+    return GRAV_OK;
+}
+
+grav_status grav_store_g(grav_ctx* c, int fp32, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    const int elem = fp32 ? 4 : 8;
+    const size_t need = c->lay.gstore + (size_t)c->g.N * c->g.M * elem;
+    if (c->ws_bytes < need) return fail(GRAV_ENOTFIT, "stored G does not fit in the workspace");
+    DeviceGuard dg(c->device);
+    c->stored_elem = 0;
+    CK(launch_tabulate(c, c->ws + c->lay.gstore, elem, (cudaStream_t)stream), "tabulate");
+    c->stored_elem = elem;
+    return GRAV_OK;
+}
+
+grav_status grav_stored_g(const grav_ctx* c, const void** gdev, int* elem) {
+    if (!c || !gdev || !elem) return fail(GRAV_EINVAL, "NULL argument");
+    *elem = c->stored_elem;
+    *gdev = c->stored_elem ? (const void*)(c->ws + c->lay.gstore) : nullptr;
+    return GRAV_OK;
+}
+
+grav_status grav_forward_stored(grav_ctx* c, const double* u, double* d, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!u || !d) return fail(GRAV_EINVAL, "NULL vector");
+    if (!c->stored_elem) return fail(GRAV_ESTATE, "no stored G (grav_store_g)");
+    DeviceGuard dg(c->device);
+    CK(launch_gemv(c, c->ws + c->lay.gstore, c->stored_elem, u, d, (cudaStream_t)stream), "gemv");
+    return GRAV_OK;
+}
+
+grav_status grav_adjoint_stored(grav_ctx* c, const double* v, double* gout, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!v || !gout) return fail(GRAV_EINVAL, "NULL vector");
+    if (!c->stored_elem) return fail(GRAV_ESTATE, "no stored G (grav_store_g)");
+    DeviceGuard dg(c->device);
+    CK(launch_gemvt(c, c->ws + c->lay.gstore, c->stored_elem, v, nullptr, gout, wsp<double>(c, c->lay.gemvt_partial),
+                    (cudaStream_t)stream), "gemvt");
+    return GRAV_OK;
+}
+
+grav_status grav_gram_diag(grav_ctx* c, const double* w, double* diag, void* stream) {
+    if (!c || !w || !diag) return fail(GRAV_EINVAL, "NULL argument");
+    DeviceGuard dg(c->device);
+    CK(launch_gram_diag(c, w, diag, (cudaStream_t)stream), "gram_diag");
+    return GRAV_OK;
+}
+
+grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, double lambda, int iters, double rtol,
+                              int mode, grav_cg_state* state, double* alpha, double* m, double* hist, double* ab,
+                              void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!dobs || !w || !alpha) return fail(GRAV_EINVAL, "NULL vector");
+    if (iters < 0 || !(lambda == lambda) || !(rtol >= 0.0)) return fail(GRAV_EINVAL, "bad iters / lambda / rtol");
+    if (mode != GRAV_MATRIX_FREE && mode != GRAV_STORED_F64 && mode != GRAV_STORED_F32)
+        return fail(GRAV_EINVAL, "bad mode");
+    if (mode != GRAV_MATRIX_FREE && c->stored_elem != (mode == GRAV_STORED_F64 ? 8 : 4))
+        return fail(GRAV_ESTATE, "stored G of the requested precision not present (grav_store_g)");
+    if (state && (!state->x_dev || !state->r_dev || !state->p_dev || !state->rho_dev))
+        return fail(GRAV_EINVAL, "NULL pointer in grav_cg_state");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const Geom& g = c->g;
+    double* x = state ? state->x_dev : wsp<double>(c, c->lay.cg_x);
+    double* r = state ? state->r_dev : wsp<double>(c, c->lay.cg_r);
+    double* p = state ? state->p_dev : wsp<double>(c, c->lay.cg_p);
+    double* q = wsp<double>(c, c->lay.cg_q);
+    double* dotA = wsp<double>(c, c->lay.dot_partial);
+    double* dotB = dotA + kDotBlocks;
+    CgScalars* sc = wsp<CgScalars>(c, c->lay.scalars);
+    double* gcell = wsp<double>(c, c->lay.gcell);
+    double* cnode = wsp<double>(c, c->lay.cnode);
+    double* tnode = wsp<double>(c, c->lay.tnode);
+    double* fpart = wsp<double>(c, c->lay.fwd_partial);
+    const void* G = c->ws + c->lay.gstore;
+    const int resume = state ? state->resume : 0;
+
+    CK(launch_cg_init(c, dobs, x, r, p, dotA, sc, rtol, resume, state ? state->rho_dev : nullptr, hist, s), "cg_init");
+    for (int it = 0; it < iters; ++it) {
+        if (mode == GRAV_MATRIX_FREE) {
+            // q = gamma^2 * Fwd( S^T W^-2 S Adj(p) ) + lambda p
+            st = adjoint_to_tnode(c, p, &sc->done, s);
+            if (st) return st;
+            CK(launch_node_to_cell(c, tnode, w, g.gamma, gcell, s), "node_to_cell");
+            CK(launch_cell_to_node(c, gcell, nullptr, cnode, s), "cell_to_node");
+            CK(launch_forward_nodes(c, cnode, fpart, &sc->done, s), "forward_nodes");
+            CK(launch_forward_reduce(c, fpart, g.gamma, lambda, p, q, dotA, sc, s), "forward_reduce");
+        } else {
+            CK(launch_gemvt(c, G, c->stored_elem, p, w, gcell, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+            CK(launch_gemv(c, G, c->stored_elem, gcell, q, s), "gemv");
+            CK(launch_dot_pq(c, p, q, lambda, q, dotA, sc, s), "dot_pq");
+        }
+        CK(launch_cg_update_xr(c, x, r, p, q, dotA, dotB, sc, it, s), "cg_update_xr");
+        CK(launch_cg_update_p(c, r, p, dotB, sc, it, rtol, hist ? hist + it + 1 : nullptr, ab ? ab + 2 * it : nullptr, s),
+           "cg_update_p");
+    }
+    if (alpha != x) CK(cudaMemcpyAsync(alpha, x, g.N * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy alpha");
+    if (state) CK(cudaMemcpyAsync(state->rho_dev, &sc->rho[iters & 1], sizeof(double), cudaMemcpyDeviceToDevice, s), "copy rho");
+    if (m) {   // m = W^-2 G^T alpha   (Eq. 11)
+        if (mode == GRAV_MATRIX_FREE) {
+            st = adjoint_to_tnode(c, x, nullptr, s);
+            if (st) return st;
+            CK(launch_node_to_cell(c, tnode, w, g.gamma, m, s), "node_to_cell");
+        } else {
+            CK(launch_gemvt(c, G, c->stored_elem, x, w, m, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+        }
+    }
+    return GRAV_OK;
+}
+
+grav_status grav_direct_solve(grav_ctx* c, const double* dobs, const double* w, double lambda, double* A,
+                              double* alpha, double* m, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!dobs || !w || !A || !alpha) return fail(GRAV_EINVAL, "NULL argument");
+    if (c->g.N > 1024) return fail(GRAV_EINVAL, "direct solve is limited to N <= 1024");
+    if (c->stored_elem != 8) return fail(GRAV_ESTATE, "direct solve needs a stored FP64 G (grav_store_g)");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const double* G = reinterpret_cast<const double*>(c->ws + c->lay.gstore);
+    CK(launch_form_A(c, G, w, lambda, A, s), "form_A");
+    CK(launch_cholesky_solve(c, A, dobs, alpha, (int)c->g.N, s), "cholesky_solve");
+    if (m) CK(launch_gemvt(c, G, 8, alpha, w, m, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+    return GRAV_OK;
+}
+
+// ---- host-buffer (end-to-end) variants ---------------------------------------------------------------------
+grav_status grav_forward_host(grav_ctx* c, const double* u_host, double* d_host, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!u_host || !d_host) return fail(GRAV_EINVAL, "NULL vector");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    double* um = wsp<double>(c, c->lay.stage_m);
+    double* dn = wsp<double>(c, c->lay.stage_n);
+    CK(cudaMemcpyAsync(um, u_host, c->g.M * sizeof(double), cudaMemcpyHostToDevice, s), "H2D u");
+    st = grav_forward(c, um, dn, stream);
+    if (st) return st;
+    CK(cudaMemcpyAsync(d_host, dn, c->g.N * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H d");
+    CK(cudaStreamSynchronize(s), "sync");
+    return GRAV_OK;
+}
+
+grav_status grav_adjoint_host(grav_ctx* c, const double* v_host, double* g_host, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!v_host || !g_host) return fail(GRAV_EINVAL, "NULL vector");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    double* gm = wsp<double>(c, c->lay.stage_m);
+    double* vn = wsp<double>(c, c->lay.stage_n);
+    CK(cudaMemcpyAsync(vn, v_host, c->g.N * sizeof(double), cudaMemcpyHostToDevice, s), "H2D v");
+    st = grav_adjoint(c, vn, gm, stream);
+    if (st) return st;
+    CK(cudaMemcpyAsync(g_host, gm, c->g.M * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H g");
+    CK(cudaStreamSynchronize(s), "sync");
+    return GRAV_OK;
+}
+
+grav_status grav_dataspace_cg_host(grav_ctx* c, const double* dobs_host, double beta, double z0, double lambda,
+                                   int iters, double rtol, int mode, double* alpha_host, double* m_host,
+                                   double* hist_host, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!dobs_host || !alpha_host) return fail(GRAV_EINVAL, "NULL vector");
+    if (iters < 0 || iters + 1 > 4096) return fail(GRAV_EINVAL, "iters must be in [0, 4095] for the host variant");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    double* w = wsp<double>(c, c->lay.cg_w);
+    double* mm = wsp<double>(c, c->lay.stage_m);
+    double* dn = wsp<double>(c, c->lay.stage_n);
+    double* hh = wsp<double>(c, c->lay.stage_hist);
+    CK(cudaMemcpyAsync(dn, dobs_host, c->g.N * sizeof(double), cudaMemcpyHostToDevice, s), "H2D dobs");
+    st = grav_depth_weights(c, beta, z0, w, stream);
+    if (st) return st;
+    // alpha is produced in the CG's own x buffer and copied out from there
+    double* x = wsp<double>(c, c->lay.cg_x);
+    st = grav_dataspace_cg(c, dn, w, lambda, iters, rtol, mode, nullptr, x, m_host ? mm : nullptr,
+                           hist_host ? hh : nullptr, nullptr, stream);
+    if (st) return st;
+    CK(cudaMemcpyAsync(alpha_host, x, c->g.N * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H alpha");
+    if (m_host) CK(cudaMemcpyAsync(m_host, mm, c->g.M * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H m");
+    if (hist_host) CK(cudaMemcpyAsync(hist_host, hh, (iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H hist");
+    CK(cudaStreamSynchronize(s), "sync");
+    return GRAV_OK;
+}
+
+}  // extern "C"
+
+// ---- FP64 pipe peak probe ----------------------------------------------------------------------------------
+namespace {
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double seed) {
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 1.0000001, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    double sres = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (sres == 12345.678) out[0] = sres;   // never true; keeps the chain alive
+}
+}  // namespace
+
+extern "C" grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* ms) {
+    if (!ninstr || !ms || iters <= 0) return fail(GRAV_EINVAL, "bad argument");
+    DeviceGuard dg(device);
+    if (!dg.ok) return fail(GRAV_ECUDA, "cudaSetDevice failed");
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, device), "cudaGetDeviceProperties");
+    double* out = nullptr;
+    CK(cudaMalloc(&out, 8), "cudaMalloc");
+    const int blocks = prop.multiProcessorCount * 8;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    dfma_probe_kernel<<<blocks, 256>>>(out, iters / 10 + 1, 1.0);   // warm-up
+    cudaEventRecord(e0);
+    dfma_probe_kernel<<<blocks, 256>>>(out, iters, 1.0);
+    cudaEventRecord(e1);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float t = 0.f;
+    cudaEventElapsedTime(&t, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    if (e != cudaSuccess) return cuda_fail(e, "dfma probe");
+    *ninstr = (double)blocks * 256.0 * 8.0 * (double)iters;
+    *ms = t;
+    return GRAV_OK;
+}

@@ -1,0 +1,101 @@
+// grav_internal.cuh -- shared declarations of the CUDA path (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/grav.h"
+
+namespace grav {
+
+// Geometry handed to every kernel by value.  Node (a,b,c) <-> flat index (a*nyp + b)*nzp + c (z fastest), so a
+// vertical node column is contiguous; "column" col = a*nyp + b.
+struct Geom {
+    int nx, ny, nz;        // cells
+    int nxp, nyp, nzp;     // nodes per axis = cells + 1
+    int ncol;              // nxp * nyp node columns
+    long long N, M, Nn;    // stations, prisms, nodes
+    const double* xn;      // device, nxp
+    const double* yn;      // device, nyp
+    const double* zn;      // device, nzp
+    const double* xo;      // device, N
+    const double* yo;
+    const double* zo;
+    double gamma;
+};
+
+// Launch plans fixed at context creation (deterministic reduction orders).
+struct Plan {
+    // forward: grid (obs tiles, node-column chunks)
+    int fwd_tpb, fwd_obs_per_thread, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
+    // adjoint: grid (node-thread blocks, station chunks)
+    int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;
+};
+
+constexpr int kDotBlocks = 256;     // block partials of the fused CG dot products
+constexpr int kDotThreads = 256;
+
+// CG scalar block (device): see cg.cu.  rho is double-buffered by iteration parity so that no kernel reads a
+// scalar another block of the same launch writes.
+struct CgScalars {
+    double rho[2];
+    double delta, a, b, dnorm2, tol2;
+    int done, iters_done;
+};
+
+struct WsLayout {
+    size_t cnode, tnode, fwd_partial, adj_partial, gcell, cg_x, cg_r, cg_p, cg_q, cg_w, dot_partial, scalars,
+        stage_m, stage_n, stage_hist, matfree_end, gemvt_partial, gstore;
+};
+
+}  // namespace grav
+
+struct grav_ctx {
+    grav::Geom g;
+    grav::Plan plan;
+    grav::WsLayout lay;
+    int device;
+    void* geom_dev;          // one allocation holding xn,yn,zn,xo,yo,zo
+    char* ws;                // caller's workspace
+    size_t ws_bytes;
+    int stored_elem;         // 0 none, 8 FP64, 4 FP32
+    long long launches;
+};
+
+namespace grav {
+
+// every launcher returns cudaGetLastError() of its launches and bumps ctx->launches
+// --- nodeops.cu
+cudaError_t launch_cell_to_node(grav_ctx* c, const double* u, const double* w_or_null, double* cnode, cudaStream_t s);
+cudaError_t launch_node_to_cell(grav_ctx* c, const double* tnode, const double* w_or_null, double scale, double* gcell,
+                                cudaStream_t s);
+cudaError_t launch_depth_weights(grav_ctx* c, double beta, double z0, double* w, cudaStream_t s);
+// --- forward.cu : partial sums of sum_n cnode[n] Psi(node_n - obs_i) into fwd_partial
+cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s);
+// d = scale * sum_chunks partial (+ lam * p if p != NULL); if dot_partial != NULL also block partials of p.d
+cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double scale, double lam, const double* p,
+                                  double* d, double* dot_partial, const CgScalars* sc, cudaStream_t s);
+// --- adjoint.cu : tnode[n] = sum_i v_i Psi(node_n - obs_i)
+cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s);
+cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s);
+// --- cg.cu
+cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp,
+                           CgScalars* sc, double rtol, int resume, const double* rho_in, double* hist, cudaStream_t s);
+cudaError_t launch_dot_pq(grav_ctx* c, const double* p, const double* q, double lam, double* q_out, double* dotp,
+                          const CgScalars* sc, cudaStream_t s);
+cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,
+                                const double* dotp_in, double* dotp_out, CgScalars* sc, int it, cudaStream_t s);
+cudaError_t launch_cg_update_p(grav_ctx* c, const double* r, double* p, const double* dotp, CgScalars* sc, int it,
+                               double rtol, double* hist_slot, double* ab_slot, cudaStream_t s);
+// --- stored.cu
+cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s);
+cudaError_t launch_gemv(grav_ctx* c, const void* G, int elem, const double* u, double* d, cudaStream_t s);
+cudaError_t launch_gemvt(grav_ctx* c, const void* G, int elem, const double* v, const double* w_or_null, double* g,
+                         double* partial, cudaStream_t s);
+cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s);
+cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double lam, double* A, cudaStream_t s);
+cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
+cudaError_t launch_scale_cells(grav_ctx* c, double* g, const double* w, cudaStream_t s);
+int gemvt_chunks(long long N);
+
+}  // namespace grav

@@ -1,0 +1,258 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the same seeded
+inputs.  Tolerances (BASELINE.json north_star):
+  forward / adjoint / stored entries : max |gpu - oracle| <= 1e-10 * max |oracle|   (reading C15: global max)
+  CG                                  : protocol P1-P5 of SURVEY.md 8(c), 1e-8 relative where well-posed
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2602_03857_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-10
+TOL_CG = 1e-8
+
+
+def relmax(a, b):
+    return float(np.abs(np.asarray(a) - np.asarray(b)).max() / np.abs(np.asarray(b)).max())
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def make_ctx(wl, mode=0):
+    from paper_2602_03857_b200 import binding
+    return binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=0, mode=mode)
+
+
+@pytest.fixture(scope="module")
+def c1(cfg1):
+    ctx = make_ctx(cfg1["wl"], mode=1)
+    yield ctx
+    ctx.close()
+
+
+# ---- operators, config 1 (full oracle) -----------------------------------------------------------------------
+def test_forward_cfg1(cfg1, c1):
+    wl, G = cfg1["wl"], cfg1["G"]
+    u_w, _, _ = wl.test_vectors()
+    for u in (np.ones(wl.M), wl.m_true, u_w):
+        ref = oracle.dense_matvec(G, u)
+        got = host(c1.forward(dev(u)))
+        assert relmax(got, ref) <= TOL_OP
+
+
+def test_adjoint_cfg1(cfg1, c1):
+    wl, G = cfg1["wl"], cfg1["G"]
+    _, v_w, v_s = wl.test_vectors()
+    for v in (cfg1["d_obs"], v_s, v_w):
+        ref = oracle.dense_rmatvec(G, v)
+        got = host(c1.adjoint(dev(v)))
+        assert relmax(got, ref) <= TOL_OP
+
+
+def test_dot_product_test_gpu(cfg1, c1):
+    wl = cfg1["wl"]
+    u, v, _ = wl.test_vectors()
+    d = host(c1.forward(dev(u)))
+    g = host(c1.adjoint(dev(v)))
+    a, b = float(d @ v), float(u @ g)
+    assert abs(a - b) <= 1e-12 * np.linalg.norm(d) * np.linalg.norm(v)
+
+
+def test_depth_weights_cfg1(cfg1, c1):
+    wl = cfg1["wl"]
+    for beta, z0 in ((2.0, 25.0), (3.0, 10.0), (0.0, 1.0)):
+        ref = oracle.depth_weights(cfg1["mesh"], beta, z0)
+        got = host(c1.depth_weights(beta, z0))
+        assert np.abs(got / ref - 1).max() <= 4e-16
+
+
+def test_gram_diag_cfg1(cfg1, c1):
+    got = host(c1.gram_diag(dev(cfg1["w"])))
+    assert np.abs(got / cfg1["diag"] - 1).max() <= 1e-11
+
+
+def test_stored_g_cfg1(cfg1, c1):
+    wl, G = cfg1["wl"], cfg1["G"]
+    u, v, _ = wl.test_vectors()
+    c1.store_g(fp32=False)
+    Gd = host(c1.stored_g())
+    assert relmax(Gd, G) <= TOL_OP
+    assert relmax(host(c1.forward_stored(dev(u))), oracle.dense_matvec(G, u)) <= TOL_OP
+    assert relmax(host(c1.adjoint_stored(dev(v))), oracle.dense_rmatvec(G, v)) <= TOL_OP
+    c1.store_g(fp32=True)
+    G32 = host(c1.stored_g())
+    assert G32.dtype == np.float32
+    assert np.array_equal(G32, Gd.astype(np.float32)) or relmax(G32, G) <= 1e-7
+    # FP32 storage error is reported, not gated at 1e-10: bounded by float rounding of the entries
+    assert relmax(host(c1.forward_stored(dev(u))), oracle.dense_matvec(G, u)) <= 2e-7
+    assert relmax(host(c1.adjoint_stored(dev(v))), oracle.dense_rmatvec(G, v)) <= 2e-7
+    c1.store_g(fp32=False)
+
+
+# ---- ragged / irregular small workloads (several tiles, ragged tails, stretched mesh, topography) -------------
+@pytest.mark.parametrize("shape", [(1, 1, 1, 1), (2, 3, 1, 5), (5, 7, 4, 23), (13, 9, 11, 301), (7, 20, 33, 130),
+                                   (3, 3, 70, 257)])
+def test_ragged_workloads(shape):
+    nx, ny, nz, nobs = shape
+    wl = workloads.make_custom(nx, ny, nz, 30.0, nobs, seed=11 + nx, topo_amp=40.0)
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    ctx = make_ctx(wl, mode=1)
+    rng = np.random.default_rng(5)
+    u, v = wl.m_true, rng.standard_normal(wl.N)
+    d_ref = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
+    g_ref = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)
+    assert relmax(host(ctx.forward(dev(u))), d_ref) <= TOL_OP
+    assert relmax(host(ctx.adjoint(dev(v))), g_ref) <= TOL_OP
+    ctx.store_g()
+    assert relmax(host(ctx.stored_g()), oracle.tabulate(mesh, wl.xo, wl.yo, wl.zo, wl.gamma)) <= TOL_OP
+    assert relmax(host(ctx.forward_stored(dev(u))), d_ref) <= TOL_OP
+    assert relmax(host(ctx.adjoint_stored(dev(v))), g_ref) <= TOL_OP
+    w = oracle.depth_weights(mesh, 2.0, wl.z0)
+    G = oracle.tabulate(mesh, wl.xo, wl.yo, wl.zo, wl.gamma)
+    assert np.abs(host(ctx.gram_diag(dev(w))) / oracle.gram_diag(G, w) - 1).max() <= 1e-10
+    ctx.close()
+
+
+def test_stations_inside_and_below_mesh():
+    """Stations below the mesh top (Z < 0 for some nodes: borehole-like) and exactly on node planes / edges:
+    principal-value atan (C3) and the guards of C6."""
+    wl = workloads.make_custom(4, 4, 4, 10.0, 6, seed=2)
+    wl.xo = np.array([5.0, 10.0, 20.0, 13.0, 0.0, -7.0])      # 10, 20, 0 are node x-planes
+    wl.yo = np.array([4.0, 8.0, 3.0, 16.0, 0.0, 50.0])        # 8, 16, 0 are node y-planes
+    wl.zo = np.array([15.0, 10.0, -2.0, 47.0, -1.0, 20.0])    # inside cells, on a node z-plane, below everything
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    ctx = make_ctx(wl)
+    u = wl.m_true
+    ref = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
+    got = host(ctx.forward(dev(u)))
+    assert np.all(np.isfinite(got))
+    assert relmax(got, ref) <= TOL_OP
+    v = np.array([1.0, -2.0, 0.5, 3.0, -1.0, 2.0])
+    assert relmax(host(ctx.adjoint(dev(v))), oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)) <= TOL_OP
+    ctx.close()
+
+
+# ---- CG, config 1: protocol P1-P5 ------------------------------------------------------------------------------
+def test_cg_cfg1_protocol(cfg1, c1):
+    from paper_2602_03857_b200 import binding
+    wl, G, w, lam, d = cfg1["wl"], cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    wd, dd = dev(w), dev(d)
+    # P2 prefix parity: first 5 iterates
+    st5, hist5, ab5 = oracle.cg(w, lam, d, 5, G=G)
+    r5 = c1.dataspace_cg(dd, wd, lam, 5)
+    assert relmax(host(r5["alpha"]), st5.x) <= TOL_CG
+    assert np.abs(host(r5["hist"]) / hist5 - 1).max() <= TOL_CG
+    assert np.abs(host(r5["ab"]) / ab5 - 1).max() <= TOL_CG
+    # P1 step parity: inject the oracle's state at j, run ONE GPU iteration
+    for j in (0, 1, 10, 49):
+        stj, _, _ = oracle.cg(w, lam, d, j, G=G)
+        nxt, _, abn = oracle.cg(w, lam, d, 1, G=G, state=stj)
+        gs = binding.CGState(wl.N, c1.device, x=stj.x, r=stj.r, p=stj.p, rho=stj.rho)
+        out = c1.dataspace_cg(dd, wd, lam, 1, state=gs, want_m=False)
+        assert np.abs(host(out["ab"])[0] / abn[0] - 1).max() <= 1e-9
+        assert relmax(host(gs.x), nxt.x) <= 1e-9
+        assert np.abs(host(gs.r) - nxt.r).max() <= 1e-9 * np.abs(d).max()
+        assert np.abs(host(gs.p) - nxt.p).max() <= 1e-9 * np.abs(d).max()
+        assert abs(float(gs.rho.item()) / nxt.rho - 1) <= 1e-8
+    # P3 converged parity: k = 50 (config's count) and k = 100 vs oracle CG and oracle Cholesky
+    alpha_dir, m_dir = oracle.dataspace_direct(G, w, lam, d)
+    st50, hist50, _ = oracle.cg(w, lam, d, 50, G=G)
+    r50 = c1.dataspace_cg(dd, wd, lam, 50)
+    assert relmax(host(r50["alpha"]), st50.x) <= TOL_CG
+    assert relmax(host(r50["alpha"]), alpha_dir) <= 5e-8      # CG truncation itself is 2.5e-9
+    assert relmax(host(r50["m"]), oracle.recover_model(G, w, st50.x)) <= TOL_CG
+    r100 = c1.dataspace_cg(dd, wd, lam, 100)
+    assert relmax(host(r100["alpha"]), alpha_dir) <= TOL_CG
+    assert relmax(host(r100["m"]), m_dir) <= TOL_CG
+    # P4 fixed-k report against the oracle's own reorder sensitivity
+    st50r, _, _ = oracle.cg(w, lam, d, 50, G=G, reverse=True)
+    self_sens = relmax(st50r.x, st50.x)
+    assert relmax(host(r50["alpha"]), st50.x) <= max(TOL_CG, 10 * self_sens)
+    # P5 invariants: true residual vs recursive residual
+    A = oracle.form_A(G, w, lam)
+    true_res = np.linalg.norm(d - A @ host(r50["alpha"])) / np.linalg.norm(d)
+    rec_res = host(r50["hist"])[-1] / np.linalg.norm(d)
+    assert abs(true_res - rec_res) <= 1e-6 * max(true_res, 1e-9) + 1e-12
+    # stored-G CG follows the same iterates
+    c1.store_g()
+    s50 = c1.dataspace_cg(dd, wd, lam, 50, mode=1)
+    assert relmax(host(s50["alpha"]), st50.x) <= TOL_CG
+    assert relmax(host(s50["m"]), oracle.recover_model(G, w, st50.x)) <= TOL_CG
+
+
+def test_cg_rtol_freeze(cfg1, c1):
+    w, lam, d = cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    out = c1.dataspace_cg(dev(d), dev(w), lam, 60, rtol=1e-6)
+    hist = host(out["hist"])
+    k = int(np.argmax(hist <= 1e-6 * hist[0]))
+    assert 0 < k < 60
+    assert np.all(hist[k:] == hist[k])            # frozen after reaching the tolerance
+    # the frozen result is exactly the k-iteration result of the same solver, and close to the oracle's k-th iterate
+    fixed = c1.dataspace_cg(dev(d), dev(w), lam, k)
+    assert np.array_equal(host(out["alpha"]), host(fixed["alpha"]))
+    assert np.array_equal(host(out["m"]), host(fixed["m"]))
+    ref, _, _ = oracle.cg(w, lam, d, k, G=cfg1["G"])
+    assert relmax(host(out["alpha"]), ref.x) <= 1e-4
+
+
+def test_direct_solve_cfg1(cfg1, c1):
+    w, lam, d = cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    c1.store_g()
+    alpha, m = c1.direct_solve(dev(d), dev(w), lam)
+    a_ref, m_ref = oracle.dataspace_direct(cfg1["G"], w, lam, d)
+    assert relmax(host(alpha), a_ref) <= TOL_CG
+    assert relmax(host(m), m_ref) <= TOL_CG
+
+
+def test_host_entry_points(cfg1, c1):
+    wl, w, lam, d = cfg1["wl"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    u, v, _ = wl.test_vectors()
+    up = torch.as_tensor(u).pin_memory()
+    dh = torch.empty(wl.N, dtype=torch.float64).pin_memory()
+    c1.forward_host(up, dh)
+    assert np.array_equal(dh.numpy(), host(c1.forward(dev(u))))
+    gh = np.empty(wl.M)
+    c1.adjoint_host(np.ascontiguousarray(v), gh)
+    assert np.array_equal(gh, host(c1.adjoint(dev(v))))
+    ah, mh, hh = np.empty(wl.N), np.empty(wl.M), np.empty(11)
+    c1.dataspace_cg_host(np.ascontiguousarray(d), wl.beta, wl.z0, lam, 10, ah, mh, hh)
+    ref = c1.dataspace_cg(dev(d), c1.depth_weights(wl.beta, wl.z0), lam, 10)
+    assert np.array_equal(ah, host(ref["alpha"])) and np.array_equal(mh, host(ref["m"]))
+    assert np.array_equal(hh, host(ref["hist"]))
+
+
+def test_determinism(cfg1, c1):
+    wl = cfg1["wl"]
+    u, v, _ = wl.test_vectors()
+    a = host(c1.forward(dev(u)))
+    b = host(c1.forward(dev(u)))
+    assert np.array_equal(a, b)
+    a = host(c1.adjoint(dev(v)))
+    b = host(c1.adjoint(dev(v)))
+    assert np.array_equal(a, b)
+
+
+def test_error_paths(cfg1, c1):
+    from paper_2602_03857_b200 import binding
+    wl = cfg1["wl"]
+    with pytest.raises(binding.GravError):
+        binding.GravContext(wl.xn[::-1].copy(), wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma)   # decreasing nodes
+    with pytest.raises(ValueError):
+        c1.forward(torch.zeros(wl.M - 1, dtype=torch.float64, device="cuda"))
+    with pytest.raises(binding.GravError):
+        c1.dataspace_cg(dev(cfg1["d_obs"]), dev(cfg1["w"]), 1.0, 3, mode=7)
+    fresh = make_ctx(wl)
+    with pytest.raises(binding.GravError) as ei:
+        fresh.forward_stored(dev(np.ones(wl.M)))
+    assert ei.value.status == -4
+    fresh.close()
