@@ -137,6 +137,17 @@ long long grav_launch_count(const grav_ctx* ctx);
  * Used to confirm the FP64 pipe peak in the same run as the roofline numbers. */
 grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* ms);
 
+/* Diagnostics.  variant 0 (default): hand-built Psi evaluator (table-driven ln, reduced-argument atan, MUFU-seeded
+ * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same kernels with CUDA libm (sqrt, /, atan, log).  Both are
+ * tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
+grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
+/* Host-side evaluation of the variant-0 algorithm (same source, MUFU seeds emulated at 2^-20 accuracy) so that
+ * CPU-only tests can check it: returns Psi(X,Y,Z) + (X+Y)*k0*ln2 (the offset cancels in every signed sum, see
+ * csrc/psi.cuh). */
+double grav_debug_psi_fast_host(double X, double Y, double Z, int k0);
+/* The global exponent offset k0 chosen for this context (2^k0 ~ survey scale). */
+int grav_debug_k0(const grav_ctx* ctx);
+
 /* Thread-local message of the last failure on this thread ("" if none). */
 const char* grav_last_error(void);
 

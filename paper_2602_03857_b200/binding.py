@@ -21,7 +21,8 @@ EXPORTS = [
     "grav_forward", "grav_adjoint", "grav_depth_weights", "grav_dataspace_cg", "grav_store_g",
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_launch_count",
-    "grav_fp64_peak_probe", "grav_last_error",
+    "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host",
+    "grav_debug_k0",
 ]
 
 
@@ -82,6 +83,12 @@ def load():
     L.grav_launch_count.argtypes = [vp]
     L.grav_fp64_peak_probe.restype = i
     L.grav_fp64_peak_probe.argtypes = [i, i, dp, dp]
+    L.grav_debug_set_psi_variant.restype = i
+    L.grav_debug_set_psi_variant.argtypes = [vp, i]
+    L.grav_debug_psi_fast_host.restype = d
+    L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
+    L.grav_debug_k0.restype = i
+    L.grav_debug_k0.argtypes = [vp]
     L.grav_last_error.restype = C.c_char_p
     L.grav_last_error.argtypes = []
     _lib = L
@@ -272,9 +279,22 @@ class GravContext:
                                                 _host(hist_host, iters + 1, "hist"), _stream()))
         return alpha_host
 
+    def set_psi_variant(self, variant):
+        """0: hand-built evaluator (default); 1: CUDA libm (cross-check)."""
+        _check(self._lib.grav_debug_set_psi_variant(self._h, int(variant)))
+
+    @property
+    def k0(self):
+        return int(self._lib.grav_debug_k0(self._h))
+
     @property
     def launches(self):
         return int(self._lib.grav_launch_count(self._h))
+
+
+def psi_fast_host(X, Y, Z, k0=0):
+    """Host emulation of the device Psi evaluator (diagnostic; needs no GPU)."""
+    return float(load().grav_debug_psi_fast_host(float(X), float(Y), float(Z), int(k0)))
 
 
 def fp64_peak_probe(device=0, iters=200000):

@@ -14,12 +14,15 @@ namespace grav {
 
 constexpr int kAdjObsTile = 256;
 
-template <int TPB, int KC>
-__global__ void __launch_bounds__(TPB) adjoint_nodes_kernel(Geom g, const double* __restrict__ v,
-                                                             double* __restrict__ partial, int ncg, int obs_per_chunk,
-                                                             const int* __restrict__ done) {
+template <int TPB, int KC, bool FAST>
+__global__ void __launch_bounds__(TPB, 512 / TPB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
+                                                                        double* __restrict__ partial, int ncg,
+                                                                        int obs_per_chunk, const int* __restrict__ done) {
+    extern __shared__ double2 s_tab[];
     if (done && *done) return;
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
+    PsiTabView tb;
+    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
     const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long nthreads = (long long)g.ncol * ncg;
     const bool valid = t < nthreads;
@@ -46,12 +49,15 @@ __global__ void __launch_bounds__(TPB) adjoint_nodes_kernel(Geom g, const double
         for (int j = 0; j < cnt; ++j) {
             const double4 o = s_obs[j];
             const double X = xa - o.x, Y = yb - o.y;
-            const double XY = X * Y;
-            const double Q = fma(Y, Y, X * X);
+            if (FAST) {
+                const PsiColumn pc = psi_column(X, Y);
 #pragma unroll
-            for (int k = 0; k < KC; ++k) {
-                const double Z = zc[k] - o.z;
-                acc[k] = fma(o.w, GRAV_PSI(X, Y, Z, XY, Q), acc[k]);
+                for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_fast(tb, pc, zc[k] - o.z), acc[k]);
+            } else {
+                const double XY = X * Y;
+                const double Q = fma(Y, Y, X * X);
+#pragma unroll
+                for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
             }
         }
     }
@@ -72,10 +78,20 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     tnode[n] = s;
 }
 
+cudaError_t init_adjoint_kernels() {
+    return cudaFuncSetAttribute(adjoint_nodes_kernel<128, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kTabSmemBytes);
+}
+
 cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
     const Plan& p = c->plan;
     dim3 grid(p.adj_blocks, p.adj_nchunk);
-    adjoint_nodes_kernel<128, 8><<<grid, 128, 0, s>>>(c->g, v, partial, p.adj_ncg, p.adj_obs_per_chunk, done);
+    if (c->psi_variant == 0)
+        adjoint_nodes_kernel<128, 8, true><<<grid, 128, kTabSmemBytes, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
+                                                                           p.adj_obs_per_chunk, done);
+    else
+        adjoint_nodes_kernel<128, 8, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
+                                                                 p.adj_obs_per_chunk, done);
     c->launches++;
     return cudaGetLastError();
 }

@@ -4,18 +4,22 @@
 //
 // Tiling: one thread owns one station (coordinates and accumulator in registers); a block owns a tile of
 // stations and a chunk of node columns; the node coefficients c_n of the chunk are read by every thread at the
-// same address (broadcast).  X, Y, X*Y and X^2+Y^2 are constant down a node column and hoisted out of the
+// same address (broadcast).  X, Y, |XY| and X^2+Y^2 are constant down a node column and hoisted out of the
 // z-loop.  Chunk partial sums go to partial[chunk][N]; forward_reduce adds them in fixed order (deterministic).
+// Bound: FP64 pipe: ~49 FP64 instructions per evaluation, 8 bytes of c_n per warp.
 #include "grav_internal.cuh"
 #include "psi.cuh"
 
 namespace grav {
 
-template <int TPB>
-__global__ void __launch_bounds__(TPB) forward_nodes_kernel(Geom g, const double* __restrict__ cnode,
-                                                             double* __restrict__ partial, int cols_per_chunk,
-                                                             const int* __restrict__ done) {
+template <int TPB, bool FAST>
+__global__ void __launch_bounds__(TPB, 512 / TPB) forward_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ cnode,
+                                                                        double* __restrict__ partial, int cols_per_chunk,
+                                                                        const int* __restrict__ done) {
+    extern __shared__ double2 s_tab[];
     if (done && *done) return;
+    PsiTabView tb;
+    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
@@ -26,14 +30,24 @@ __global__ void __launch_bounds__(TPB) forward_nodes_kernel(Geom g, const double
     double X = __ldg(g.xn + a) - xo;
     for (int col = col0; col < col1; ++col) {
         const double Y = __ldg(g.yn + b) - yo;
-        const double XY = X * Y;
-        const double Q = fma(Y, Y, X * X);
         const double* __restrict__ cc = cnode + (long long)col * g.nzp;
         double colacc = 0.0;
-        for (int c = 0; c < g.nzp; ++c) {
-            const double Z = __ldg(g.zn + c) - zo;
-            const double coef = __ldg(cc + c);
-            colacc = fma(coef, GRAV_PSI(X, Y, Z, XY, Q), colacc);
+        if (FAST) {
+            const PsiColumn pc = psi_column(X, Y);
+#pragma unroll 2
+            for (int c = 0; c < g.nzp; ++c) {
+                const double Z = __ldg(g.zn + c) - zo;
+                const double coef = __ldg(cc + c);
+                colacc = fma(coef, psi_fast(tb, pc, Z), colacc);
+            }
+        } else {
+            const double XY = X * Y;
+            const double Q = fma(Y, Y, X * X);
+            for (int c = 0; c < g.nzp; ++c) {
+                const double Z = __ldg(g.zn + c) - zo;
+                const double coef = __ldg(cc + c);
+                colacc = fma(coef, psi_libm(X, Y, Z, XY, Q), colacc);
+            }
         }
         acc += colacc;
         if (++b == g.nyp) {
@@ -76,10 +90,18 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
     }
 }
 
+cudaError_t init_forward_kernels() {
+    return cudaFuncSetAttribute(forward_nodes_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kTabSmemBytes);
+}
+
 cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
     const Plan& p = c->plan;
     dim3 grid(p.fwd_tiles, p.fwd_nchunk);
-    forward_nodes_kernel<128><<<grid, 128, 0, s>>>(c->g, cnode, partial, p.fwd_cols_per_chunk, done);
+    if (c->psi_variant == 0)
+        forward_nodes_kernel<128, true><<<grid, 128, kTabSmemBytes, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
+    else
+        forward_nodes_kernel<128, false><<<grid, 128, 0, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
     c->launches++;
     return cudaGetLastError();
 }

@@ -158,7 +158,8 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     g.gamma = gamma;
     c->device = device;
 
-    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + 6 * 32;   // each array 256-byte aligned
+    const size_t ntab = sizeof(PsiTablesHost) / sizeof(double);
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + 7 * 32;   // each array 256-byte aligned
     std::vector<double> host;
     try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
     void* dev = nullptr;
@@ -173,9 +174,28 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     };
     g.xn = put(xn, g.nxp); g.yn = put(yn, g.nyp); g.zn = put(zn, g.nzp);
     g.xo = put(ox, nobs); g.yo = put(oy, nobs); g.zo = put(oz, nobs);
+    {   // Psi tables (csrc/psi.cuh) and the global exponent offset: 2^k0 ~ half the horizontal survey diagonal
+        PsiTablesHost tabs;
+        psi_tables_generate(&tabs);
+        c->pd.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs), ntab));
+        double lox = xn[0], hix = xn[nx], loy = yn[0], hiy = yn[ny];
+        for (long long i = 0; i < nobs; ++i) {
+            lox = ox[i] < lox ? ox[i] : lox; hix = ox[i] > hix ? ox[i] : hix;
+            loy = oy[i] < loy ? oy[i] : loy; hiy = oy[i] > hiy ? oy[i] : hiy;
+        }
+        const double diag = std::sqrt((hix - lox) * (hix - lox) + (hiy - loy) * (hiy - loy));
+        c->pd.k0 = (diag > 0.0 && std::isfinite(diag)) ? (int)std::ilogb(0.5 * diag) : 0;
+        if (c->pd.k0 > 900) c->pd.k0 = 900;
+        if (c->pd.k0 < -900) c->pd.k0 = -900;
+        c->psi_variant = 0;
+    }
     e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaMemcpy geometry"); }
     c->geom_dev = dev;
+    e = init_forward_kernels();
+    if (e == cudaSuccess) e = init_adjoint_kernels();
+    if (e == cudaSuccess) e = init_stored_kernels();
+    if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaFuncSetAttribute"); }
     make_plan(g, c->plan);
     make_layout(g, c->plan, c->lay);
     *out = c;
@@ -214,6 +234,24 @@ grav_status grav_set_workspace(grav_ctx* c, void* ws, size_t bytes) {
 }
 
 long long grav_launch_count(const grav_ctx* c) { return c ? c->launches : 0; }
+
+grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {
+    if (!c || (variant != 0 && variant != 1)) return fail(GRAV_EINVAL, "bad context / variant");
+    c->psi_variant = variant;
+    c->stored_elem = 0;
+    return GRAV_OK;
+}
+
+int grav_debug_k0(const grav_ctx* c) { return c ? c->pd.k0 : 0; }
+
+double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
+    static PsiTablesHost tabs;
+    static bool ready = false;
+    if (!ready) { psi_tables_generate(&tabs); ready = true; }
+    PsiTabView tb;
+    tb.base = tabs.e; tb.shift = 0; tb.k0 = k0;
+    return psi_fast(tb, psi_column(X, Y), Z);
+}
 
 grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {
     grav_status st = check_ready(c);

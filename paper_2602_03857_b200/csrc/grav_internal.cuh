@@ -5,6 +5,7 @@
 #include <stdint.h>
 
 #include "../../include/grav.h"
+#include "psi.cuh"
 
 namespace grav {
 
@@ -59,6 +60,8 @@ struct grav_ctx {
     char* ws;                // caller's workspace
     size_t ws_bytes;
     int stored_elem;         // 0 none, 8 FP64, 4 FP32
+    grav::PsiDev pd;         // Psi tables (inside geom_dev) and the global exponent offset k0
+    int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
     long long launches;
 };
 
@@ -97,5 +100,8 @@ cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double 
 cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
 cudaError_t launch_scale_cells(grav_ctx* c, double* g, const double* w, cudaStream_t s);
 int gemvt_chunks(long long N);
+cudaError_t init_forward_kernels();
+cudaError_t init_adjoint_kernels();
+cudaError_t init_stored_kernels();
 
 }  // namespace grav

@@ -17,14 +17,9 @@ namespace grav {
 // ---- per-pair evaluation ---------------------------------------------------------------------------------
 // Flattened "layer" index q = cc*nzp + c over cell columns cc = i*ny + j and node layers c = 0..nz.
 // A warp owns 32 consecutive q starting at 31*warp; lane l < 31 outputs the prism (cc, k=c) if c < nz.
-struct PairLane {
-    long long q;     // layer index (clamped)
-    int cc, c;       // cell column, layer
-    bool has_prism;  // this lane's (cc, c) is a prism and the next lane holds layer c+1 of the same column
-};
-
-__device__ __forceinline__ double layer_value(const Geom& g, long long q, long long nq, double xo, double yo, double zo,
-                                              int& cc, int& c) {
+template <bool FAST>
+__device__ __forceinline__ double layer_value(const Geom& g, const PsiTabView& tb, long long q, long long nq, double xo,
+                                              double yo, double zo, int& cc, int& c) {
     q = q < nq ? q : nq - 1;
     cc = (int)(q / g.nzp);
     c = (int)(q - (long long)cc * g.nzp);
@@ -33,15 +28,26 @@ __device__ __forceinline__ double layer_value(const Geom& g, long long q, long l
     const double Y1 = g.yn[j] - yo, Y2 = g.yn[j + 1] - yo;
     const double Z = g.zn[c] - zo;
     // (-1)^(da+db): (0,0)+, (1,0)-, (0,1)-, (1,1)+
-    double v = GRAV_PSI(X1, Y1, Z, X1 * Y1, fma(Y1, Y1, X1 * X1));
-    v -= GRAV_PSI(X2, Y1, Z, X2 * Y1, fma(Y1, Y1, X2 * X2));
-    v -= GRAV_PSI(X1, Y2, Z, X1 * Y2, fma(Y2, Y2, X1 * X1));
-    v += GRAV_PSI(X2, Y2, Z, X2 * Y2, fma(Y2, Y2, X2 * X2));
+    double v;
+    if (FAST) {
+        v = psi_fast(tb, psi_column(X1, Y1), Z);
+        v -= psi_fast(tb, psi_column(X2, Y1), Z);
+        v -= psi_fast(tb, psi_column(X1, Y2), Z);
+        v += psi_fast(tb, psi_column(X2, Y2), Z);
+    } else {
+        v = psi_libm(X1, Y1, Z, X1 * Y1, fma(Y1, Y1, X1 * X1));
+        v -= psi_libm(X2, Y1, Z, X2 * Y1, fma(Y1, Y1, X2 * X2));
+        v -= psi_libm(X1, Y2, Z, X1 * Y2, fma(Y2, Y2, X1 * X1));
+        v += psi_libm(X2, Y2, Z, X2 * Y2, fma(Y2, Y2, X2 * X2));
+    }
     return v;
 }
 
-template <typename T, int TPB>
-__global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, T* __restrict__ G) {
+template <typename T, int TPB, bool FAST>
+__global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, PsiDev pd, T* __restrict__ G) {
+    extern __shared__ double2 s_tab[];
+    PsiTabView tb;
+    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
     const long long nq = (long long)g.nx * g.ny * g.nzp;
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * TPB + threadIdx.x) >> 5;
@@ -49,7 +55,7 @@ __global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, T* __restrict__ G
     if (warp * 31 >= nq) return;
     for (long long i = blockIdx.y; i < g.N; i += gridDim.y) {
         int cc, c;
-        const double L = layer_value(g, q, nq, g.xo[i], g.yo[i], g.zo[i], cc, c);
+        const double L = layer_value<FAST>(g, tb, q, nq, g.xo[i], g.yo[i], g.zo[i], cc, c);
         const double Lnext = __shfl_down_sync(0xffffffffu, L, 1);
         if (lane < 31 && q < nq && c < g.nz) {
             const long long m = (long long)cc * g.nz + c;
@@ -58,10 +64,13 @@ __global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, T* __restrict__ G
     }
 }
 
-template <int TPB>
-__global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, const double* __restrict__ w,
+template <int TPB, bool FAST>
+__global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, PsiDev pd, const double* __restrict__ w,
                                                          double* __restrict__ diag) {
+    extern __shared__ double2 s_tab[];
     __shared__ double sh[TPB];
+    PsiTabView tb;
+    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
     const long long nq = (long long)g.nx * g.ny * g.nzp;
     const int lane = threadIdx.x & 31;
     const int warp_in_block = threadIdx.x >> 5;
@@ -73,7 +82,7 @@ __global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, const double* __
         for (long long wt = warp_in_block; wt < nwarp_tasks; wt += WPB) {
             const long long q = wt * 31 + lane;
             int cc, c;
-            const double L = layer_value(g, q, nq, xo, yo, zo, cc, c);
+            const double L = layer_value<FAST>(g, tb, q, nq, xo, yo, zo, cc, c);
             const double Lnext = __shfl_down_sync(0xffffffffu, L, 1);
             if (lane < 31 && q < nq && c < g.nz) {
                 const double gv = g.gamma * (Lnext - L);
@@ -263,17 +272,30 @@ static unsigned pair_blocks(const Geom& g, int tpb) {
     return (unsigned)((nwarps * 32 + tpb - 1) / tpb);
 }
 
+cudaError_t init_stored_kernels() {
+    cudaError_t e = cudaFuncSetAttribute(tabulate_kernel<double, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tabulate_kernel<float, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gram_diag_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+    return e;
+}
+
 cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
     dim3 grid(pair_blocks(c->g, 256), (unsigned)(c->g.N < 65535 ? c->g.N : 65535));
-    if (elem == 8) tabulate_kernel<double, 256><<<grid, 256, 0, s>>>(c->g, (double*)G);
-    else tabulate_kernel<float, 256><<<grid, 256, 0, s>>>(c->g, (float*)G);
+    if (c->psi_variant == 0) {
+        if (elem == 8) tabulate_kernel<double, 256, true><<<grid, 256, kTabSmemBytes, s>>>(c->g, c->pd, (double*)G);
+        else tabulate_kernel<float, 256, true><<<grid, 256, kTabSmemBytes, s>>>(c->g, c->pd, (float*)G);
+    } else {
+        if (elem == 8) tabulate_kernel<double, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd, (double*)G);
+        else tabulate_kernel<float, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd, (float*)G);
+    }
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
     unsigned blocks = (unsigned)(c->g.N < (1 << 20) ? c->g.N : (1 << 20));
-    gram_diag_kernel<256><<<blocks, 256, 0, s>>>(c->g, w, diag);
+    if (c->psi_variant == 0) gram_diag_kernel<256, true><<<blocks, 256, kTabSmemBytes, s>>>(c->g, c->pd, w, diag);
+    else gram_diag_kernel<256, false><<<blocks, 256, 0, s>>>(c->g, c->pd, w, diag);
     c->launches++;
     return cudaGetLastError();
 }

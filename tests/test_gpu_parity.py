@@ -256,3 +256,16 @@ def test_error_paths(cfg1, c1):
         fresh.forward_stored(dev(np.ones(wl.M)))
     assert ei.value.status == -4
     fresh.close()
+
+
+def test_libm_variant_matches(cfg1):
+    """The CUDA-libm evaluator (variant 1) and the hand-built one (variant 0, default) both match the oracle."""
+    wl, G = cfg1["wl"], cfg1["G"]
+    u, v, _ = wl.test_vectors()
+    ctx = make_ctx(wl, mode=1)
+    ctx.set_psi_variant(1)
+    assert relmax(host(ctx.forward(dev(u))), oracle.dense_matvec(G, u)) <= TOL_OP
+    assert relmax(host(ctx.adjoint(dev(v))), oracle.dense_rmatvec(G, v)) <= TOL_OP
+    ctx.store_g()
+    assert relmax(host(ctx.stored_g()), G) <= TOL_OP
+    ctx.close()
