@@ -141,6 +141,9 @@ grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* 
  * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same kernels with CUDA libm (sqrt, /, atan, log).  Both are
  * tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
 grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
+/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel; value: variant index,
+ * 0 = default).  Every variant computes the same sums in the same order per thread. */
+grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
 /* Host-side evaluation of the variant-0 algorithm (same source, MUFU seeds emulated at 2^-20 accuracy) so that
  * CPU-only tests can check it: returns Psi(X,Y,Z) + (X+Y)*k0*ln2 (the offset cancels in every signed sum, see
  * csrc/psi.cuh). */

@@ -22,7 +22,7 @@ EXPORTS = [
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_launch_count",
     "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host",
-    "grav_debug_k0",
+    "grav_debug_k0", "grav_debug_set_tuning",
 ]
 
 
@@ -87,6 +87,8 @@ def load():
     L.grav_debug_set_psi_variant.argtypes = [vp, i]
     L.grav_debug_psi_fast_host.restype = d
     L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
+    L.grav_debug_set_tuning.restype = i
+    L.grav_debug_set_tuning.argtypes = [vp, i, i]
     L.grav_debug_k0.restype = i
     L.grav_debug_k0.argtypes = [vp]
     L.grav_last_error.restype = C.c_char_p
@@ -282,6 +284,9 @@ class GravContext:
     def set_psi_variant(self, variant):
         """0: hand-built evaluator (default); 1: CUDA libm (cross-check)."""
         _check(self._lib.grav_debug_set_psi_variant(self._h, int(variant)))
+
+    def set_tuning(self, which, value):
+        _check(self._lib.grav_debug_set_tuning(self._h, int(which), int(value)))
 
     @property
     def k0(self):

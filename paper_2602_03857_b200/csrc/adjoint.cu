@@ -14,8 +14,8 @@ namespace grav {
 
 constexpr int kAdjObsTile = 256;
 
-template <int TPB, int KC, bool FAST>
-__global__ void __launch_bounds__(TPB, 512 / TPB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
+template <int TPB, int KC, int MINB, bool FAST>
+__global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
                                                                         double* __restrict__ partial, int ncg,
                                                                         int obs_per_chunk, const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
@@ -51,8 +51,9 @@ __global__ void __launch_bounds__(TPB, 512 / TPB) adjoint_nodes_kernel(Geom g, P
             const double X = xa - o.x, Y = yb - o.y;
             if (FAST) {
                 const PsiColumn pc = psi_column(X, Y);
+                const double vs = o.w * pc.s;
 #pragma unroll
-                for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_fast(tb, pc, zc[k] - o.z), acc[k]);
+                for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_fast(tb, pc, zc[k] - o.z), acc[k]);
             } else {
                 const double XY = X * Y;
                 const double Q = fma(Y, Y, X * X);
@@ -78,22 +79,48 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     tnode[n] = s;
 }
 
-cudaError_t init_adjoint_kernels() {
-    return cudaFuncSetAttribute(adjoint_nodes_kernel<128, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kTabSmemBytes);
+template <int TPB, int KC, int MINB>
+static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
+    static bool inited = false;
+    if (!inited) {
+        cudaError_t e = cudaFuncSetAttribute(adjoint_nodes_kernel<TPB, KC, MINB, true>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+        if (e != cudaSuccess) return e;
+        inited = true;
+    }
+    const Plan& p = c->plan;
+    const int ncg = (c->g.nzp + KC - 1) / KC;
+    const long long nthreads = (long long)c->g.ncol * ncg;
+    dim3 grid((unsigned)((nthreads + TPB - 1) / TPB), p.adj_nchunk);
+    adjoint_nodes_kernel<TPB, KC, MINB, true><<<grid, TPB, kTabSmemBytes, s>>>(c->g, c->pd, v, partial, ncg,
+                                                                              p.adj_obs_per_chunk, done);
+    return cudaGetLastError();
 }
+
+cudaError_t init_adjoint_kernels() { return cudaSuccess; }
 
 cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
     const Plan& p = c->plan;
-    dim3 grid(p.adj_blocks, p.adj_nchunk);
-    if (c->psi_variant == 0)
-        adjoint_nodes_kernel<128, 8, true><<<grid, 128, kTabSmemBytes, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
-                                                                           p.adj_obs_per_chunk, done);
-    else
-        adjoint_nodes_kernel<128, 8, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
-                                                                 p.adj_obs_per_chunk, done);
+    cudaError_t e;
+    if (c->psi_variant == 0) {
+        switch (c->tune[1]) {
+            default:
+            case 0: e = adj_launch_fast<128, 8, 4>(c, v, partial, done, s); break;
+            case 1: e = adj_launch_fast<256, 4, 3>(c, v, partial, done, s); break;
+            case 2: e = adj_launch_fast<256, 8, 2>(c, v, partial, done, s); break;
+            case 3: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
+            case 4: e = adj_launch_fast<256, 2, 3>(c, v, partial, done, s); break;
+            case 5: e = adj_launch_fast<256, 4, 2>(c, v, partial, done, s); break;
+            case 6: e = adj_launch_fast<256, 2, 4>(c, v, partial, done, s); break;
+        }
+    } else {
+        dim3 grid(p.adj_blocks, p.adj_nchunk);
+        adjoint_nodes_kernel<128, 8, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
+                                                                    p.adj_obs_per_chunk, done);
+        e = cudaGetLastError();
+    }
     c->launches++;
-    return cudaGetLastError();
+    return e;
 }
 
 cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s) {

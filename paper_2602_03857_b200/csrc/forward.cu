@@ -12,8 +12,8 @@
 
 namespace grav {
 
-template <int TPB, bool FAST>
-__global__ void __launch_bounds__(TPB, 512 / TPB) forward_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ cnode,
+template <int TPB, int UNROLL, int MINB, bool FAST>
+__global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ cnode,
                                                                         double* __restrict__ partial, int cols_per_chunk,
                                                                         const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
@@ -34,12 +34,13 @@ __global__ void __launch_bounds__(TPB, 512 / TPB) forward_nodes_kernel(Geom g, P
         double colacc = 0.0;
         if (FAST) {
             const PsiColumn pc = psi_column(X, Y);
-#pragma unroll 2
+#pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
                 const double Z = __ldg(g.zn + c) - zo;
                 const double coef = __ldg(cc + c);
                 colacc = fma(coef, psi_fast(tb, pc, Z), colacc);
             }
+            colacc *= pc.s;
         } else {
             const double XY = X * Y;
             const double Q = fma(Y, Y, X * X);
@@ -90,20 +91,46 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
     }
 }
 
-cudaError_t init_forward_kernels() {
-    return cudaFuncSetAttribute(forward_nodes_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)kTabSmemBytes);
+// Launch variants (grav_debug_set_tuning(ctx, 0, v)); the default is the one measured fastest (profiles/).
+template <int TPB, int UNROLL, int MINB>
+static cudaError_t fwd_launch_fast(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
+    static bool inited = false;
+    if (!inited) {
+        cudaError_t e = cudaFuncSetAttribute(forward_nodes_kernel<TPB, UNROLL, MINB, true>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+        if (e != cudaSuccess) return e;
+        inited = true;
+    }
+    const Plan& p = c->plan;
+    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);
+    forward_nodes_kernel<TPB, UNROLL, MINB, true><<<grid, TPB, kTabSmemBytes, s>>>(c->g, c->pd, cnode, partial,
+                                                                                  p.fwd_cols_per_chunk, done);
+    return cudaGetLastError();
 }
+
+cudaError_t init_forward_kernels() { return cudaSuccess; }
 
 cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
     const Plan& p = c->plan;
-    dim3 grid(p.fwd_tiles, p.fwd_nchunk);
-    if (c->psi_variant == 0)
-        forward_nodes_kernel<128, true><<<grid, 128, kTabSmemBytes, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
-    else
-        forward_nodes_kernel<128, false><<<grid, 128, 0, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
+    cudaError_t e;
+    if (c->psi_variant == 0) {
+        switch (c->tune[0]) {
+            default:
+            case 0: e = fwd_launch_fast<128, 2, 4>(c, cnode, partial, done, s); break;
+            case 1: e = fwd_launch_fast<256, 1, 3>(c, cnode, partial, done, s); break;
+            case 2: e = fwd_launch_fast<256, 2, 2>(c, cnode, partial, done, s); break;
+            case 3: e = fwd_launch_fast<128, 1, 4>(c, cnode, partial, done, s); break;
+            case 4: e = fwd_launch_fast<256, 1, 4>(c, cnode, partial, done, s); break;
+            case 5: e = fwd_launch_fast<256, 4, 2>(c, cnode, partial, done, s); break;
+            case 6: e = fwd_launch_fast<512, 2, 1>(c, cnode, partial, done, s); break;
+        }
+    } else {
+        dim3 grid(p.fwd_tiles, p.fwd_nchunk);
+        forward_nodes_kernel<128, 1, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
+        e = cudaGetLastError();
+    }
     c->launches++;
-    return cudaGetLastError();
+    return e;
 }
 
 cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double scale, double lam, const double* p,

@@ -187,6 +187,7 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         c->pd.k0 = (diag > 0.0 && std::isfinite(diag)) ? (int)std::ilogb(0.5 * diag) : 0;
         if (c->pd.k0 > 900) c->pd.k0 = 900;
         if (c->pd.k0 < -900) c->pd.k0 = -900;
+        c->pd.k = psi_consts_make(c->pd.k0);
         c->psi_variant = 0;
     }
     e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
@@ -242,6 +243,12 @@ grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {
     return GRAV_OK;
 }
 
+grav_status grav_debug_set_tuning(grav_ctx* c, int which, int value) {
+    if (!c || which < 0 || which >= 4) return fail(GRAV_EINVAL, "bad context / selector");
+    c->tune[which] = value;
+    return GRAV_OK;
+}
+
 int grav_debug_k0(const grav_ctx* c) { return c ? c->pd.k0 : 0; }
 
 double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
@@ -249,8 +256,9 @@ double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
     static bool ready = false;
     if (!ready) { psi_tables_generate(&tabs); ready = true; }
     PsiTabView tb;
-    tb.base = tabs.e; tb.shift = 0; tb.k0 = k0;
-    return psi_fast(tb, psi_column(X, Y), Z);
+    tb.base = tabs.e; tb.shift = 0; tb.k = psi_consts_make(k0); tb.ik = psi_int_consts(0);
+    const PsiColumn pc = psi_column(X, Y);
+    return pc.s * psi_fast(tb, pc, Z);
 }
 
 grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {

@@ -62,6 +62,7 @@ struct grav_ctx {
     int stored_elem;         // 0 none, 8 FP64, 4 FP32
     grav::PsiDev pd;         // Psi tables (inside geom_dev) and the global exponent offset k0
     int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
+    int tune[4];             // launch-variant selectors (grav_debug_set_tuning): 0 forward, 1 adjoint
     long long launches;
 };
 

@@ -30,10 +30,12 @@ __device__ __forceinline__ double layer_value(const Geom& g, const PsiTabView& t
     // (-1)^(da+db): (0,0)+, (1,0)-, (0,1)-, (1,1)+
     double v;
     if (FAST) {
-        v = psi_fast(tb, psi_column(X1, Y1), Z);
-        v -= psi_fast(tb, psi_column(X2, Y1), Z);
-        v -= psi_fast(tb, psi_column(X1, Y2), Z);
-        v += psi_fast(tb, psi_column(X2, Y2), Z);
+        const PsiColumn c11 = psi_column(X1, Y1), c21 = psi_column(X2, Y1), c12 = psi_column(X1, Y2),
+                        c22 = psi_column(X2, Y2);
+        v = c11.s * psi_fast(tb, c11, Z);
+        v = fma(-c21.s, psi_fast(tb, c21, Z), v);
+        v = fma(-c12.s, psi_fast(tb, c12, Z), v);
+        v = fma(c22.s, psi_fast(tb, c22, Z), v);
     } else {
         v = psi_libm(X1, Y1, Z, X1 * Y1, fma(Y1, Y1, X1 * X1));
         v -= psi_libm(X2, Y1, Z, X2 * Y1, fma(Y1, Y1, X2 * X2));
