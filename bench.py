@@ -30,7 +30,9 @@ UNIT = "pair evals/s"
 
 # FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
 # capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
-FP64_INST_PER_EVAL = {"forward_nodes": 116.0, "adjoint_nodes": 116.0}
+FP64_INST_PER_EVAL = {"forward_nodes": 48.0, "adjoint_nodes": 49.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture (profiles/)
+NCU_DRAM_BYTES = {"forward_nodes": None, "adjoint_nodes": None}
 FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
 
 
@@ -172,27 +174,33 @@ def run_reference(args):
 def run_ours(args):
     import torch
     from paper_2602_03857_b200 import binding, workloads
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        from paper_2602_03857_b200 import dist as gdist
-        return gdist.bench_sharded(args, METRIC, UNIT)
+    from paper_2602_03857_b200 import dist as gdist
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    rank, world, local = gdist.init_from_env("nccl")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     wl = workloads.make(args.config)
     N, M, Nn = wl.N, wl.M, wl.n_nodes
-    ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+    # observation-sharded over the ranks; world == 1: the whole station set, no exchange hook
+    sh = gdist.ShardedContext(wl, rank, world, local)
+    ctx, Nloc = sh.ctx, sh.hi - sh.lo
     to = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+            torch.cuda.synchronize()
 
     # ---- inputs resident in HBM: d_obs = G m_true + noise (GPU forward, parity-checked in tests/), weights, lambda
     w = ctx.depth_weights(wl.beta, wl.z0)
     d_clean = ctx.forward(to(wl.m_true))
-    sigma = wl.noise_frac * float(d_clean.abs().max().item())
-    d_obs = d_clean + sigma * to(wl.noise())
+    dmax = d_clean.abs().max().reshape(1)
+    if world > 1:
+        torch.distributed.all_reduce(dmax, op=torch.distributed.ReduceOp.MAX)
+    sigma = wl.noise_frac * float(dmax.item())
+    d_obs = d_clean + sigma * sh.local(wl.noise())
     # lambda = 1e-2 * trace / N, trace/N estimated as the mean Gram diagonal over <= 512 seeded stations
     nsub = min(N, 512)
     idx = np.sort(np.random.default_rng(3).choice(N, size=nsub, replace=False))
@@ -202,7 +210,7 @@ def run_ours(args):
 
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    state = binding.CGState(N, dev)
+    state = binding.CGState(Nloc, dev)
 
     def one_step(first):
         state.resume = not first
@@ -211,27 +219,26 @@ def run_ours(args):
     # ---- warm-up, then K timed steps (L2 flushed between steps, CUDA events on the launching stream)
     for k in range(args.warmup):
         one_step(k == 0)
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
     launches0 = ctx.launches
-    times = []
+    total_ms = 0.0
     for k in range(args.steps):
         flush.fill_(k & 0xFF)
         e0, e1 = ev(), ev()
-        torch.cuda.synchronize()
+        barrier()
         e0.record()
         one_step(args.warmup == 0 and k == 0)
         e1.record()
-        torch.cuda.synchronize()
-        times.append(e0.elapsed_time(e1))
+        barrier()
+        total_ms += gdist.max_over_ranks(e0.elapsed_time(e1), dev)
     launches = ctx.launches - launches0
-    total_ms = sum(times)
     pairs_per_step = 2.0 * N * M
     value = pairs_per_step * args.steps / (total_ms * 1e-3)
 
     # ---- the two dominant kernels timed alone (same launch configuration), for the roofline object
     u_vec = to(wl.m_true)
-    dn, gm = torch.empty(N, dtype=torch.float64, device=dev), torch.empty(M, dtype=torch.float64, device=dev)
+    dn, gm = torch.empty(Nloc, dtype=torch.float64, device=dev), torch.empty(M, dtype=torch.float64, device=dev)
 
     def timed(fn, reps):
         fn()
@@ -239,34 +246,34 @@ def run_ours(args):
         for _ in range(reps):
             flush.fill_(1)
             e0, e1 = ev(), ev()
-            torch.cuda.synchronize()
+            barrier()
             e0.record(); fn(); e1.record()
-            torch.cuda.synchronize()
+            barrier()
             ts.append(e0.elapsed_time(e1))
         return statistics.median(ts)
 
     reps = max(1, min(3, args.steps))
     t_fwd = timed(lambda: ctx.forward(u_vec, out=dn), reps)
     t_adj = timed(lambda: ctx.adjoint(d_obs, out=gm), reps)
-    clocks = sampler.stop()
+    clocks = sampler.stop() if sampler else None
 
-    evals = float(N) * Nn
+    evals = float(Nloc) * Nn                     # node evaluations one launch of this rank processes
     dom, t_dom = ("forward_nodes", t_fwd) if t_fwd >= t_adj else ("adjoint_nodes", t_adj)
     inst = FP64_INST_PER_EVAL[dom] * evals
     achieved = inst / (t_dom * 1e-3) / 1e12
     peak_nominal = 148 * FP64_LANES_PER_SM * 1.965e9 / 1e12
     probe_rate, _ = binding.fp64_peak_probe(local, 100000)
-    clk = clocks.get("sm_mhz") or 1965.0
+    clk = (clocks or {}).get("sm_mhz") or 1965.0
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_nominal,
-        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": None,
-        "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz (nominal, DESIGN.md); DFMA probe in this run: "
-                       f"{probe_rate / 1e12:.2f} T inst/s",
+        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": NCU_DRAM_BYTES.get(dom),
+        "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz = 1 DFMA/DMUL/DADD per lane per clock (DESIGN.md 6); "
+                       f"DFMA-only probe in this run: {probe_rate / 1e12:.2f} T inst/s",
         "frac_of_probe": achieved / (probe_rate / 1e12),
         "frac_at_held_clock": achieved / (148 * FP64_LANES_PER_SM * clk * 1e6 / 1e12),
         "fp64_inst_per_eval": FP64_INST_PER_EVAL[dom], "evals_per_launch": evals,
         "ms_forward": t_fwd, "ms_adjoint": t_adj,
-        "pairs_per_s_forward": N * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": N * M / (t_adj * 1e-3),
+        "pairs_per_s_forward": float(Nloc) * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": float(Nloc) * M / (t_adj * 1e-3),
     }
 
     # ---- end to end through the host-buffer C-ABI call: H2D d_obs, weights, 1 CG iteration + model recovery,
@@ -274,35 +281,44 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         dh = d_obs.cpu().pin_memory()
-        ah = torch.empty(N, dtype=torch.float64).pin_memory()
+        ah = torch.empty(Nloc, dtype=torch.float64).pin_memory()
         mh = torch.empty(M, dtype=torch.float64).pin_memory()
         ctx.dataspace_cg_host(dh, wl.beta, wl.z0, lam, 1, ah, mh)      # warm
         nrep = max(1, min(args.steps, 3))
+        barrier()
         t0 = time.perf_counter()
         for _ in range(nrep):
             ctx.dataspace_cg_host(dh, wl.beta, wl.z0, lam, 1, ah, mh)
-        dt = time.perf_counter() - t0
-        e2e = {"value": 3.0 * N * M * nrep / dt, "unit": UNIT, "h2d_bytes_per_step": 8 * N,
-               "d2h_bytes_per_step": 8 * (N + M), "ms_per_step": 1e3 * dt / nrep,
+        barrier()
+        dt = gdist.max_over_ranks((time.perf_counter() - t0) * 1e3, dev) * 1e-3
+        e2e = {"value": 3.0 * N * M * nrep / dt, "unit": UNIT, "h2d_bytes_per_step": 8 * Nloc,
+               "d2h_bytes_per_step": 8 * (Nloc + M), "ms_per_step": 1e3 * dt / nrep,
                "call": "grav_dataspace_cg_host(iters=1): H2D d_obs, depth weights, 1 CG iteration (adjoint+forward) "
-                       "+ model recovery (adjoint) = 3*N*M pairs, D2H alpha+m"}
+                       "+ model recovery (adjoint) = 3*N*M pairs, D2H alpha+m; host wall clock around the "
+                       "synchronising call, bytes per rank"}
 
     cpu = None
-    if not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_oracle_rate(wl, args.cpu_seconds)
 
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": total_ms / args.steps, "s_per_cg_iter": total_ms / args.steps * 1e-3,
-        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wl.name, "prisms": M, "stations": N, "nodes": Nn, "pairs_per_step": pairs_per_step,
-                   "step": "one data-space CG iteration (G^T p, W^-2, G(.), fused vector ops)",
-                   "l2": "flushed between steps (256 MiB write)", "lambda": lam,
-                   "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-    }
-    print(json.dumps(line))
-    ctx.close()
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+            "s_per_cg_iter": total_ms / args.steps * 1e-3, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "prisms": M, "stations": N, "nodes": Nn,
+                       "pairs_per_step": pairs_per_step,
+                       "step": "one data-space CG iteration (G^T p, W^-2, G(.), fused vector ops)",
+                       "parallelism": f"stations sharded over {world} rank(s); all-reduce of node sums + dot partials",
+                       "l2": "flushed between steps (256 MiB write)", "lambda": lam,
+                       "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    sh.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
 
 
 def main():

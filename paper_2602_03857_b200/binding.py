@@ -22,8 +22,11 @@ EXPORTS = [
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_launch_count",
     "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host",
-    "grav_debug_k0", "grav_debug_set_tuning",
+    "grav_debug_k0", "grav_debug_set_tuning", "grav_set_allreduce",
 ]
+
+# int fn(double* buf_dev, long long count, void* stream, void* user)   (include/grav.h: grav_allreduce_fn)
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p)
 
 
 class GravError(RuntimeError):
@@ -89,6 +92,8 @@ def load():
     L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
     L.grav_debug_set_tuning.restype = i
     L.grav_debug_set_tuning.argtypes = [vp, i, i]
+    L.grav_set_allreduce.restype = i
+    L.grav_set_allreduce.argtypes = [vp, ALLREDUCE_FN, vp]
     L.grav_debug_k0.restype = i
     L.grav_debug_k0.argtypes = [vp]
     L.grav_last_error.restype = C.c_char_p
@@ -280,6 +285,27 @@ class GravContext:
                                                 _host(alpha_host, self.N, "alpha"), _host(m_host, self.M, "m"),
                                                 _host(hist_host, iters + 1, "hist"), _stream()))
         return alpha_host
+
+    def set_allreduce(self, fn):
+        """Register the observation-sharding exchange hook (include/grav.h: grav_set_allreduce).
+        fn(ptr: int, count: int, stream: int) -> None sums `count` doubles at device address `ptr` over all ranks,
+        in place, ordered on the CUDA stream `stream`; None restores single-rank operation."""
+        if fn is None:
+            self._hook = None
+            _check(self._lib.grav_set_allreduce(self._h, C.cast(None, ALLREDUCE_FN), None))
+            return
+
+        def tramp(buf, count, stream, user):
+            try:
+                fn(int(buf), int(count), int(stream or 0))
+                return 0
+            except Exception:           # no exception may cross the C ABI
+                import traceback
+                traceback.print_exc()
+                return 1
+
+        self._hook = ALLREDUCE_FN(tramp)      # keep the trampoline alive as long as the context uses it
+        _check(self._lib.grav_set_allreduce(self._h, self._hook, None))
 
     def set_psi_variant(self, variant):
         """0: hand-built evaluator (default); 1: CUDA libm (cross-check)."""

@@ -105,17 +105,17 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
     if (c->psi_variant == 0) {
         switch (c->tune[1]) {
             default:
-            case 0: e = adj_launch_fast<128, 8, 4>(c, v, partial, done, s); break;
+            case 0: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
             case 1: e = adj_launch_fast<256, 4, 3>(c, v, partial, done, s); break;
             case 2: e = adj_launch_fast<256, 8, 2>(c, v, partial, done, s); break;
-            case 3: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
+            case 3: e = adj_launch_fast<128, 8, 4>(c, v, partial, done, s); break;
             case 4: e = adj_launch_fast<256, 2, 3>(c, v, partial, done, s); break;
             case 5: e = adj_launch_fast<256, 4, 2>(c, v, partial, done, s); break;
             case 6: e = adj_launch_fast<256, 2, 4>(c, v, partial, done, s); break;
         }
     } else {
         dim3 grid(p.adj_blocks, p.adj_nchunk);
-        adjoint_nodes_kernel<128, 8, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
+        adjoint_nodes_kernel<128, 4, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
                                                                     p.adj_obs_per_chunk, done);
         e = cudaGetLastError();
     }

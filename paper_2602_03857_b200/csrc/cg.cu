@@ -135,11 +135,17 @@ __global__ void cg_check_done_kernel(CgScalars* sc, int it) {
     if (!sc->done && sc->tol2 > 0.0 && sc->rho[(it + 1) & 1] <= sc->tol2) sc->done = 1;
 }
 
-cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp,
-                           CgScalars* sc, double rtol, int resume, const double* rho_in, double* hist, cudaStream_t s) {
+cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp, int resume,
+                           cudaStream_t s) {
     cg_init_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, dobs, x, r, p, dotp, resume);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc, double rtol, int resume,
+                                  const double* rho_in, double* hist, cudaStream_t s) {
     cg_init_finish_kernel<<<1, kDotThreads, 0, s>>>(dotp, sc, rtol, resume, rho_in, hist);
-    c->launches += 2;
+    c->launches++;
     return cudaGetLastError();
 }
 

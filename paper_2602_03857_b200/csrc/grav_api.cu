@@ -47,7 +47,7 @@ void make_plan(const Geom& g, Plan& p) {
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
     p.adj_tpb = 128;
-    p.adj_kc = 8;
+    p.adj_kc = 4;
     p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
     want = ceil_div(target_blocks, p.adj_blocks);
@@ -101,7 +101,15 @@ struct DeviceGuard {
     ~DeviceGuard() { cudaSetDevice(prev); }
 };
 
-// node sums T = sum_i v_i Psi(node - obs_i) into ws.tnode
+// Observation-sharded operation (grav_set_allreduce): sum `count` doubles at `buf` over all ranks, in place, ordered
+// on stream `s`.  No-op for a single-rank context.
+grav_status exchange(grav_ctx* c, double* buf, long long count, cudaStream_t s) {
+    if (!c->allreduce) return GRAV_OK;
+    if (c->allreduce(buf, count, (void*)s, c->allreduce_user) != 0) return fail(GRAV_ECUDA, "all-reduce hook failed");
+    return GRAV_OK;
+}
+
+// node sums T = sum_i v_i Psi(node - obs_i) into ws.tnode (summed over ranks when sharded)
 grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cudaStream_t s) {
     double* part = wsp<double>(c, c->lay.adj_partial);
     double* tn = wsp<double>(c, c->lay.tnode);
@@ -111,7 +119,7 @@ grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cuda
         CK(launch_adjoint_nodes(c, v, part, done, s), "adjoint_nodes");
         CK(launch_adjoint_reduce(c, part, tn, s), "adjoint_reduce");
     }
-    return GRAV_OK;
+    return exchange(c, tn, c->g.Nn, s);
 }
 
 }  // namespace
@@ -234,6 +242,13 @@ grav_status grav_set_workspace(grav_ctx* c, void* ws, size_t bytes) {
     return GRAV_OK;
 }
 
+grav_status grav_set_allreduce(grav_ctx* c, grav_allreduce_fn fn, void* user) {
+    if (!c) return fail(GRAV_EINVAL, "NULL context");
+    c->allreduce = fn;
+    c->allreduce_user = user;
+    return GRAV_OK;
+}
+
 long long grav_launch_count(const grav_ctx* c) { return c ? c->launches : 0; }
 
 grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {
@@ -341,7 +356,7 @@ grav_status grav_adjoint_stored(grav_ctx* c, const double* v, double* gout, void
     DeviceGuard dg(c->device);
     CK(launch_gemvt(c, c->ws + c->lay.gstore, c->stored_elem, v, nullptr, gout, wsp<double>(c, c->lay.gemvt_partial),
                     (cudaStream_t)stream), "gemvt");
-    return GRAV_OK;
+    return exchange(c, gout, c->g.M, (cudaStream_t)stream);
 }
 
 grav_status grav_gram_diag(grav_ctx* c, const double* w, double* diag, void* stream) {
@@ -381,7 +396,9 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
     const void* G = c->ws + c->lay.gstore;
     const int resume = state ? state->resume : 0;
 
-    CK(launch_cg_init(c, dobs, x, r, p, dotA, sc, rtol, resume, state ? state->rho_dev : nullptr, hist, s), "cg_init");
+    CK(launch_cg_init(c, dobs, x, r, p, dotA, resume, s), "cg_init");
+    if ((st = exchange(c, dotA, kDotBlocks, s))) return st;
+    CK(launch_cg_init_finish(c, dotA, sc, rtol, resume, state ? state->rho_dev : nullptr, hist, s), "cg_init_finish");
     for (int it = 0; it < iters; ++it) {
         if (mode == GRAV_MATRIX_FREE) {
             // q = gamma^2 * Fwd( S^T W^-2 S Adj(p) ) + lambda p
@@ -393,10 +410,13 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
             CK(launch_forward_reduce(c, fpart, g.gamma, lambda, p, q, dotA, sc, s), "forward_reduce");
         } else {
             CK(launch_gemvt(c, G, c->stored_elem, p, w, gcell, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+            if ((st = exchange(c, gcell, g.M, s))) return st;
             CK(launch_gemv(c, G, c->stored_elem, gcell, q, s), "gemv");
             CK(launch_dot_pq(c, p, q, lambda, q, dotA, sc, s), "dot_pq");
         }
+        if ((st = exchange(c, dotA, kDotBlocks, s))) return st;
         CK(launch_cg_update_xr(c, x, r, p, q, dotA, dotB, sc, it, s), "cg_update_xr");
+        if ((st = exchange(c, dotB, kDotBlocks, s))) return st;
         CK(launch_cg_update_p(c, r, p, dotB, sc, it, rtol, hist ? hist + it + 1 : nullptr, ab ? ab + 2 * it : nullptr, s),
            "cg_update_p");
     }
@@ -409,6 +429,7 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
             CK(launch_node_to_cell(c, tnode, w, g.gamma, m, s), "node_to_cell");
         } else {
             CK(launch_gemvt(c, G, c->stored_elem, x, w, m, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+            if ((st = exchange(c, m, g.M, s))) return st;
         }
     }
     return GRAV_OK;
@@ -421,6 +442,7 @@ grav_status grav_direct_solve(grav_ctx* c, const double* dobs, const double* w, 
     if (!dobs || !w || !A || !alpha) return fail(GRAV_EINVAL, "NULL argument");
     if (c->g.N > 1024) return fail(GRAV_EINVAL, "direct solve is limited to N <= 1024");
     if (c->stored_elem != 8) return fail(GRAV_ESTATE, "direct solve needs a stored FP64 G (grav_store_g)");
+    if (c->allreduce) return fail(GRAV_ESTATE, "direct solve is not available on an observation-sharded context");
     DeviceGuard dg(c->device);
     cudaStream_t s = (cudaStream_t)stream;
     const double* G = reinterpret_cast<const double*>(c->ws + c->lay.gstore);

@@ -63,6 +63,8 @@ struct grav_ctx {
     grav::PsiDev pd;         // Psi tables (inside geom_dev) and the global exponent offset k0
     int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
     int tune[4];             // launch-variant selectors (grav_debug_set_tuning): 0 forward, 1 adjoint
+    grav_allreduce_fn allreduce;   // observation-sharded operation: sum over ranks (NULL = single rank)
+    void* allreduce_user;
     long long launches;
 };
 
@@ -83,8 +85,10 @@ cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double sca
 cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s);
 cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s);
 // --- cg.cu
-cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp,
-                           CgScalars* sc, double rtol, int resume, const double* rho_in, double* hist, cudaStream_t s);
+cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp, int resume,
+                           cudaStream_t s);
+cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc, double rtol, int resume,
+                                  const double* rho_in, double* hist, cudaStream_t s);
 cudaError_t launch_dot_pq(grav_ctx* c, const double* p, const double* q, double lam, double* q_out, double* dotp,
                           const CgScalars* sc, cudaStream_t s);
 cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,

@@ -1,0 +1,110 @@
+"""Observation-sharded operation over several GPUs of one node (one process per GPU, torch.distributed / NCCL).
+
+The path shards the way the paper shards it ("observation domain partitioned across devices,
+model-space variables replicated and synchronised"): rank r owns a contiguous block of stations and the whole mesh.
+  forward  d = G u      : rows of d are local -- no communication;
+  adjoint  g = G^T v    : every rank forms the node sums T over ITS stations, one all-reduce(sum) of T (N_n doubles,
+                          27 MB at config 5) makes them global -- the only data-path collective;
+  CG                    : alpha, x, r, p, q are station vectors (local rows); each dot product all-reduces its 256
+                          block partials, so every rank computes bit-identical scalars on the device.
+The exchanges are issued by libgrav.so itself through the hook of include/grav.h (grav_set_allreduce); this module
+only provides the hook (an NCCL all-reduce on a tensor view of the buffer) and the station partition.  Nothing here
+computes any part of the method.
+"""
+import os
+
+import numpy as np
+import torch
+import torch.distributed as dist
+
+
+def shard_range(n: int, world: int, rank: int):
+    """Contiguous, balanced partition of range(n): the first n % world ranks get one extra item."""
+    if world <= 0 or not (0 <= rank < world):
+        raise ValueError("bad world / rank")
+    base, extra = divmod(n, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+class _RawDeviceArray:
+    """Zero-copy view of `count` doubles at a raw CUDA address (CUDA array interface, consumed by torch.as_tensor)."""
+
+    def __init__(self, ptr, count):
+        self.__cuda_array_interface__ = {"shape": (int(count),), "typestr": "<f8", "data": (int(ptr), False),
+                                         "version": 2}
+
+
+class AllReduceHook:
+    """Callable for GravContext.set_allreduce: sums `count` doubles at a raw address, in place, over `group`.
+
+    device = a CUDA device: the buffer is viewed zero-copy as a float64 tensor and reduced with NCCL; the collective
+    is ordered after the work already enqueued on the current stream and the current stream waits for it (torch's
+    synchronous all_reduce semantics), which is the stream libgrav.so was given.
+    device = "cpu": host address (gloo; used by the CPU tests of this plumbing)."""
+
+    def __init__(self, device, group=None):
+        self.device = torch.device(device)
+        self.group = group
+        self.calls = 0
+        self.elements = 0
+
+    def view(self, ptr: int, count: int) -> torch.Tensor:
+        if self.device.type == "cuda":
+            return torch.as_tensor(_RawDeviceArray(ptr, count), device=self.device)
+        import ctypes
+        return torch.from_numpy(np.ctypeslib.as_array((ctypes.c_double * count).from_address(ptr)))
+
+    def __call__(self, ptr: int, count: int, stream: int = 0):
+        v = self.view(ptr, count)
+        dist.all_reduce(v, op=dist.ReduceOp.SUM, group=self.group)
+        self.calls += 1
+        self.elements += count
+
+
+def init_from_env(backend="nccl"):
+    """torchrun environment -> (rank, world, local_rank); initialises the default process group once."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29500")
+        if backend == "nccl":
+            torch.cuda.set_device(local)
+            dist.init_process_group(backend, rank=rank, world_size=world, device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend, rank=rank, world_size=world)
+    return rank, world, local
+
+
+class ShardedContext:
+    """GravContext on this rank's station shard with the exchange hook installed."""
+
+    def __init__(self, wl, rank, world, local, mode=0):
+        from . import binding
+        self.rank, self.world = rank, world
+        self.lo, self.hi = shard_range(wl.N, world, rank)
+        sl = slice(self.lo, self.hi)
+        self.ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo[sl], wl.yo[sl], wl.zo[sl], wl.gamma, device=local,
+                                       mode=mode)
+        self.hook = None
+        if world > 1:
+            self.hook = AllReduceHook(self.ctx.device)
+            self.ctx.set_allreduce(self.hook)
+
+    def local(self, a):
+        """Rows of a station vector (numpy) owned by this rank, as a device tensor."""
+        return torch.as_tensor(np.ascontiguousarray(a[self.lo:self.hi], dtype=np.float64)).to(self.ctx.device)
+
+    def close(self):
+        self.ctx.close()
+
+
+def max_over_ranks(ms: float, device) -> float:
+    """Device-timed milliseconds -> max over ranks (the contract's multi-GPU timing rule)."""
+    if not dist.is_initialized():
+        return ms
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())

@@ -1,0 +1,184 @@
+"""GPU parity at BASELINE.json's full sizes (configs 2-5), in the launch configuration bench.py times.
+
+The oracle cannot run a whole product at these sizes (config 5: ~80 core-hours), so parity is closed by
+(SURVEY.md 8(c) pins):
+  * sampled outputs the oracle computes one by one: forward on seeded stations x ALL prisms, adjoint on seeded
+    prisms x ALL stations (footprint corners, extreme topography, top / bottom layers included);
+  * properties that hold at any size and touch every pair: whole-mesh row sums (forward(u = 1) equals the gz of
+    ONE prism, the mesh bounding box, 8 oracle evaluations per station), the dot-product test <G u, v> = <u, G^T v>;
+  * CG: hybrid prefix parity (the oracle's CG arithmetic restated in numpy long double around grav_forward /
+    grav_adjoint), true-vs-recursive residual; config 2 additionally converged parity against a Cholesky solve of
+    the oracle's explicit A.
+Tolerance: 1e-10 of the global max of the output (reading C15).  For white-noise adjoint inputs the FP64 oracle's
+own cancellation error reaches ~2e-10 at config-5 scale; there the gate is the error against the
+long-double build of the oracle: gpu_err <= max(1e-10, 2 x oracle_f64_err).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2602_03857_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-10
+TOL_CG = 1e-8
+LD = np.longdouble
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+class Case:
+    """One configuration: workload, context, oracle mesh, sampled stations / cells, shared device vectors."""
+
+    def __init__(self, cfg):
+        from paper_2602_03857_b200 import binding
+        self.cfg = cfg
+        self.wl = wl = workloads.make(cfg)
+        self.mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+        self.ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=0)
+        rng = np.random.default_rng(1000 + cfg)
+        ns = {2: 256, 3: 256, 4: 192, 5: 128}[cfg]
+        # stations: seeded sample + the extremes (footprint corners, highest / lowest station)
+        r2 = lambda cx, cy: (wl.xo - cx) ** 2 + (wl.yo - cy) ** 2
+        Lx, Ly = wl.xn[-1], wl.yn[-1]
+        ext = [int(np.argmin(r2(0, 0))), int(np.argmin(r2(Lx, 0))), int(np.argmin(r2(0, Ly))),
+               int(np.argmin(r2(Lx, Ly))), int(np.argmin(r2(Lx / 2, Ly / 2))), int(np.argmin(wl.zo)),
+               int(np.argmax(wl.zo)), 0, wl.N - 1]
+        self.sidx = np.unique(np.concatenate([rng.choice(wl.N, size=ns, replace=False), ext]))
+        # cells: seeded sample + mesh corners in the top and bottom layers + a centre column
+        nx, ny, nz = wl.nx, wl.ny, wl.nz
+        flat = lambda i, j, k: (i * ny + j) * nz + k
+        extc = [flat(i, j, k) for i in (0, nx - 1) for j in (0, ny - 1) for k in (0, nz - 1)]
+        extc += [flat(nx // 2, ny // 2, k) for k in (0, 1, nz // 2, nz - 1)]
+        self.cidx = np.unique(np.concatenate([rng.choice(wl.M, size=1024, replace=False), extc])).astype(np.int64)
+        self.u_w, self.v_w, self.v_s = wl.test_vectors()
+
+    def close(self):
+        self.ctx.close()
+
+
+_cases = {}
+
+
+@pytest.fixture(scope="module", params=[2, 3, 4, 5])
+def case(request):
+    cfg = request.param
+    for k in list(_cases):                      # one configuration resident at a time (config 5 is ~0.5 GB)
+        if k != cfg:
+            _cases.pop(k).close()
+    if cfg not in _cases:
+        _cases[cfg] = Case(cfg)
+    return _cases[cfg]
+
+
+def relmax(a, b, scale=None):
+    scale = np.abs(b).max() if scale is None else scale
+    return float(np.abs(np.asarray(a) - np.asarray(b)).max() / scale)
+
+
+def test_forward_sampled_stations(case):
+    wl, s = case.wl, case.sidx
+    for u in (wl.m_true, case.u_w):
+        got = host(case.ctx.forward(dev(u)))
+        ref = oracle.forward(case.mesh, wl.xo[s], wl.yo[s], wl.zo[s], wl.gamma, u)
+        assert np.all(np.isfinite(got))
+        assert relmax(got[s], ref, np.abs(got).max()) <= TOL_OP
+
+
+def test_forward_whole_mesh_row_sums(case):
+    """forward(u = 1)_i is the gz of the mesh bounding box as ONE prism (exact regrouping of all N*M pairs)."""
+    wl = case.wl
+    got = host(case.ctx.forward(dev(np.ones(wl.M))))
+    box = oracle.Mesh(wl.xn[[0, -1]], wl.yn[[0, -1]], wl.zn[[0, -1]])
+    ref = oracle.forward(box, wl.xo, wl.yo, wl.zo, wl.gamma, np.ones(1))
+    assert relmax(got, ref) <= TOL_OP
+
+
+def test_adjoint_sampled_cells(case):
+    wl, c = case.wl, case.cidx
+    for v, white in ((case.v_s, False), (case.v_w, True)):
+        got = host(case.ctx.adjoint(dev(v)))
+        assert np.all(np.isfinite(got))
+        scale = np.abs(got).max()
+        ref = oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=c)
+        err = relmax(got[c], ref, scale)
+        if err > TOL_OP and white:
+            truth = oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=c, prec=1)
+            err_gpu, err_orc = relmax(got[c], truth, scale), relmax(ref, truth, scale)
+            assert err_gpu <= max(TOL_OP, 2.0 * err_orc), (err_gpu, err_orc)
+        else:
+            assert err <= TOL_OP, err
+
+
+def test_dot_product_full_size(case):
+    """<G u, v> = <u, G^T v> ties the adjoint to the forward over every pair."""
+    u, v = case.u_w, case.v_w
+    d = host(case.ctx.forward(dev(u))).astype(LD)
+    g = host(case.ctx.adjoint(dev(v))).astype(LD)
+    a, b = float(d @ v.astype(LD)), float(u.astype(LD) @ g)
+    assert abs(a - b) <= 1e-11 * float(np.linalg.norm(d) * np.linalg.norm(v))
+
+
+def _hybrid_cg(ctx, d, w, lam, iters):
+    """The oracle's CG (oracle.cpp orc_cg: textbook Hestenes-Stiefel, x0 = 0) restated with numpy long-double
+    scalars around the device operators; returns (x, hist)."""
+    winv2 = 1.0 / (w * w)
+    x = np.zeros_like(d)
+    r, p = d.copy(), d.copy()
+    rho = float(r.astype(LD) @ r.astype(LD))
+    hist = [np.sqrt(rho)]
+    for _ in range(iters):
+        g = host(ctx.adjoint(dev(p))) * winv2
+        q = host(ctx.forward(dev(g))) + lam * p
+        a = rho / float(p.astype(LD) @ q.astype(LD))
+        x = x + a * p
+        r = r - a * q
+        rho_new = float(r.astype(LD) @ r.astype(LD))
+        p = r + (rho_new / rho) * p
+        rho = rho_new
+        hist.append(np.sqrt(rho))
+    return x, np.array(hist)
+
+
+def test_cg_prefix_and_residual(case):
+    wl, ctx = case.wl, case.ctx
+    its = 3
+    w = ctx.depth_weights(wl.beta, wl.z0)
+    wh = host(w)
+    assert np.abs(wh / oracle.depth_weights(case.mesh, wl.beta, wl.z0) - 1).max() <= 4e-16
+    d_clean = host(ctx.forward(dev(wl.m_true)))
+    d = d_clean + wl.noise_frac * np.abs(d_clean).max() * wl.noise()
+    # lambda: 1e-2 * mean Gram diagonal over sampled stations (a number handed to both solvers)
+    from paper_2602_03857_b200 import binding
+    s = case.sidx
+    sub = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo[s], wl.yo[s], wl.zo[s], wl.gamma, device=0)
+    diag = host(sub.gram_diag(w))
+    sub.close()
+    lam = wl.lam_factor * float(diag.mean())
+    out = ctx.dataspace_cg(dev(d), w, lam, its)
+    xh, hh = _hybrid_cg(ctx, d, wh, lam, its)
+    assert np.abs(host(out["hist"]) / hh - 1).max() <= TOL_CG
+    assert relmax(host(out["alpha"]), xh) <= TOL_CG
+    # true residual of the device solution equals its recursive residual
+    alpha = host(out["alpha"])
+    Aalpha = host(ctx.forward(dev(host(ctx.adjoint(dev(alpha))) / (wh * wh)))) + lam * alpha
+    true_res = np.linalg.norm(d - Aalpha) / np.linalg.norm(d)
+    rec_res = host(out["hist"])[-1] / np.linalg.norm(d)
+    assert abs(true_res - rec_res) <= 1e-6 * true_res
+    # model recovery m = W^-2 G^T alpha on sampled cells against the oracle
+    c = case.cidx
+    m_ref = oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, alpha, cells=c) / (wh[c] ** 2)
+    m = host(out["m"])
+    assert relmax(m[c], m_ref, np.abs(m).max()) <= TOL_CG
+    # Gram diagonal on the sampled stations against per-prism oracle rows (first 8 stations)
+    s8 = s[:8]
+    G8 = oracle.tabulate(case.mesh, wl.xo[s8], wl.yo[s8], wl.zo[s8], wl.gamma)
+    assert np.abs(diag[:8] / oracle.gram_diag(G8, wh) - 1).max() <= 1e-10

@@ -269,3 +269,52 @@ def test_libm_variant_matches(cfg1):
     ctx.store_g()
     assert relmax(host(ctx.stored_g()), G) <= TOL_OP
     ctx.close()
+
+
+def test_allreduce_hook_placement(cfg1):
+    """Observation sharding (include/grav.h: grav_set_allreduce).  Two IDENTICAL ranks, each holding the same
+    stations S, form the global system [G_S; G_S]; its all-reduce is "multiply by 2".  By symmetry the sharded CG must
+    then reproduce the single-rank CG of the problem with gamma*sqrt(2) (A = 2 G W^-2 G^T + lambda I): same alpha,
+    residual history and model larger by sqrt(2).  Every exchange point has to be hooked for this to hold."""
+    from paper_2602_03857_b200 import binding, dist as gdist
+    wl, w, lam, d = cfg1["wl"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    calls = []
+
+    def make_hook(ctx):
+        view = gdist.AllReduceHook(ctx.device).view
+
+        def hook(ptr, count, stream):
+            calls.append(count)
+            view(ptr, count).mul_(2.0)          # sum over two identical ranks, on the current stream
+        return hook
+
+    its = 8
+    for mode in (0, 1):
+        sh = make_ctx(wl, mode=mode)
+        sh.set_allreduce(make_hook(sh))
+        ref = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma * np.sqrt(2.0), device=0,
+                                  mode=mode)
+        if mode == 1:
+            sh.store_g()
+            ref.store_g()
+        calls.clear()
+        a = sh.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
+        b = ref.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
+        assert relmax(host(a["alpha"]), host(b["alpha"])) <= 1e-10
+        assert np.abs(host(a["hist"]) / (np.sqrt(2.0) * host(b["hist"])) - 1).max() <= 1e-10
+        assert relmax(host(a["m"]), np.sqrt(2.0) * host(b["m"])) <= 1e-10
+        big = wl.n_nodes if mode == 0 else wl.M
+        # d.d, then per iteration: operator output, p.q, r.r; finally the model recovery
+        assert calls == [256] + [big, 256, 256] * its + [big]
+        # the adjoint is global (summed over the two ranks), the forward stays local
+        v = cfg1["d_obs"]
+        calls.clear()
+        g2 = host(sh.adjoint(dev(v)) if mode == 0 else sh.adjoint_stored(dev(v)))
+        assert calls == [big]
+        sh.set_allreduce(None)
+        g1 = host(sh.adjoint(dev(v)) if mode == 0 else sh.adjoint_stored(dev(v)))
+        assert np.array_equal(g2, 2.0 * g1) and len(calls) == 1
+        with_hook_fwd = host(sh.forward(dev(wl.m_true)))
+        assert relmax(with_hook_fwd, np.sqrt(0.5) * host(ref.forward(dev(wl.m_true)))) <= 1e-13
+        sh.close()
+        ref.close()
