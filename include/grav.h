@@ -134,8 +134,8 @@ grav_status grav_dataspace_cg_host(grav_ctx* ctx, const double* dobs_host, doubl
  * variables replicated and synchronised").  Each rank creates its context on ITS OWN station shard (same mesh) and
  * registers a hook that sums `count` doubles at `buf_dev` over all ranks, in place, ordered on `stream` (e.g. an NCCL
  * all-reduce; return 0 on success).  The library calls it exactly where the method exchanges data:
- *   - the node sums T (N_n doubles) after the local adjoint kernel      -> grav_adjoint / CG / model recovery return
- *     the GLOBAL G^T v, m;   (stored modes: the M-vector after the local G^T product)
+ *   - the node sums T (2 N_n doubles: [hi | lo] planes of the compensated sums) after the local adjoint kernel
+ *     -> grav_adjoint / CG / model recovery return the GLOBAL G^T v, m;   (stored modes: the M-vector after the local G^T product)
  *   - the 256 block partials of each CG dot product (d.d, p.q, r.r)      -> every rank holds bit-identical scalars.
  * grav_forward, grav_gram_diag and alpha stay local to the rank's stations; there is no other communication.
  * fn = NULL restores single-rank operation.  grav_direct_solve is not available on a sharded context. */

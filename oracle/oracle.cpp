@@ -298,6 +298,24 @@ int orc_modelspace_direct(long long N, long long M, const double* G, const doubl
     return orc_cholesky_solve(M, B.data(), rhs.data(), m);
 }
 
+// Variant of the two dense products used ONLY for the self-sensitivity figure of protocol P4:
+// the same sums in reversed index order with a plain `double` accumulator -- a second, equally valid FP64
+// evaluation order whose results differ from the long-double-accumulated ones by ~sqrt(n)*2^-53.
+static void dense_matvec_alt(long long N, long long M, const double* G, const double* u, double* d, int nthreads) {
+    parallel_for(N, nthreads, [&](long long i) {
+        double acc = 0;
+        for (long long c = M - 1; c >= 0; --c) acc += G[i * M + c] * u[c];
+        d[i] = acc;
+    });
+}
+static void dense_rmatvec_alt(long long N, long long M, const double* G, const double* v, double* g, int nthreads) {
+    parallel_for(M, nthreads, [&](long long c) {
+        double acc = 0;
+        for (long long i = N - 1; i >= 0; --i) acc += G[i * M + c] * v[i];
+        g[c] = acc;
+    });
+}
+
 // ---- conjugate gradients on A = G W^-2 G^T + lambda I (reading C8) ----------
 // State (x, r, p, rho) is in/out so that single steps can be injected (SURVEY.md 8(c) protocol P1).
 // If `start` != 0 the state is initialised to x=0, r=p=dobs, rho=r.r first.
@@ -305,7 +323,9 @@ int orc_modelspace_direct(long long N, long long M, const double* G, const doubl
 // (mesh/station arrays required); otherwise the tabulated G is reused.
 // hist (may be NULL) receives ||r||_2 after each iteration at hist[it+1]; hist[0] = initial ||r||.
 // ab (may be NULL) receives the step scalars a_j, b_j at ab[2*it], ab[2*it+1].
-// reverse != 0 sums the dot products in reversed index order (self-sensitivity figure of protocol P4).
+// reverse != 0 (needs G): every sum (the two dense products and the dot products) runs in reversed index order
+// with a plain double accumulator -- a second valid FP64 evaluation of the same iteration.  The distance between
+// the reverse=0 and reverse=1 iterates is the oracle's own reorder sensitivity (protocol P4).
 void orc_cg(long long N, long long M, const double* G, int nx, int ny, int nz, const double* xn, const double* yn,
             const double* zn, const double* xo, const double* yo, const double* zo, double gamma, const double* w,
             double lambda, const double* dobs, int iters, int start, double* x, double* r, double* p, double* rho_io,
@@ -314,15 +334,21 @@ void orc_cg(long long N, long long M, const double* G, int nx, int ny, int nz, c
     std::vector<double> g(M), q(N);
     auto dot = [&](const double* a, const double* b) {
         ld acc = 0;
-        if (!reverse) for (long long i = 0; i < N; ++i) acc += (ld)a[i] * (ld)b[i];
-        else for (long long i = N - 1; i >= 0; --i) acc += (ld)a[i] * (ld)b[i];
-        return (double)acc;
+        if (!reverse) {
+            for (long long i = 0; i < N; ++i) acc += (ld)a[i] * (ld)b[i];
+            return (double)acc;
+        }
+        double accd = 0;
+        for (long long i = N - 1; i >= 0; --i) accd += a[i] * b[i];
+        return accd;
     };
     auto applyA = [&](const double* pin, double* qout) {
-        if (G) orc_dense_rmatvec(N, M, G, pin, g.data(), nthreads);
+        if (G && reverse) dense_rmatvec_alt(N, M, G, pin, g.data(), nthreads);
+        else if (G) orc_dense_rmatvec(N, M, G, pin, g.data(), nthreads);
         else adjoint_t<double>(mesh, N, xo, yo, zo, gamma, pin, M, nullptr, g.data(), nthreads);
         for (long long c = 0; c < M; ++c) g[c] /= (w[c] * w[c]);
-        if (G) orc_dense_matvec(N, M, G, g.data(), qout, nthreads);
+        if (G && reverse) dense_matvec_alt(N, M, G, g.data(), qout, nthreads);
+        else if (G) orc_dense_matvec(N, M, G, g.data(), qout, nthreads);
         else forward_t<double>(mesh, N, xo, yo, zo, gamma, g.data(), qout, nthreads);
         for (long long i = 0; i < N; ++i) qout[i] += lambda * pin[i];
     };

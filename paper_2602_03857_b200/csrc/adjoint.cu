@@ -5,14 +5,30 @@
 // Transposed tiling: one thread owns KC consecutive nodes of one node column (their z and accumulators live in
 // registers); stations are staged through shared memory in tiles and read at the same address by every thread
 // (broadcast).  X, Y, X*Y, X^2+Y^2 are computed once per (thread, station) and shared by the KC nodes.
-// Every node is owned by exactly one thread: no atomics.  Station chunks give partial[chunk][Nn], added in
-// fixed order by adjoint_reduce.
+// Every node is owned by exactly one thread: no atomics.
+//
+// Accumulation.  T_n is a sum of up to N same-sign terms of size |v Psi| ~ 1e4..1e5 m whose 8-corner signed
+// difference (node_to_cell) is 1e6..1e7 times smaller, so a plain running sum over all stations loses the result
+// (measured 7e-9 of max at config 5 with a smooth v).  The sum is therefore two-level: a plain FP64 running sum
+// over one tile of kAdjObsTile stations, then an error-free TwoSum (Knuth) of the tile sum into a (hi, lo) pair
+// kept in the output buffer (L2-resident; read-modify-written once per tile by the owning thread).  T is handed on
+// as two planes [hi | lo] of Nn doubles each; station chunks give partial[chunk][2][Nn], combined in fixed order
+// by adjoint_reduce with the same TwoSum.
 #include "grav_internal.cuh"
 #include "psi.cuh"
 
 namespace grav {
 
 constexpr int kAdjObsTile = 256;
+
+// (hi_out, lo_out) = (hi_in, lo_in) + x with the rounding error of hi_in + x captured exactly (Knuth TwoSum).
+__device__ __forceinline__ void two_sum_acc(double hi_in, double lo_in, double x, double& hi_out, double& lo_out) {
+    const double s = hi_in + x;
+    const double bb = s - hi_in;
+    const double err = (hi_in - (s - bb)) + (x - bb);
+    hi_out = s;
+    lo_out = lo_in + err;
+}
 
 template <int TPB, int KC, int MINB, bool FAST>
 __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
@@ -40,6 +56,8 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     }
     const long long i0 = (long long)blockIdx.y * obs_per_chunk;
     const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
+    double* out_hi = partial + (long long)blockIdx.y * 2 * g.Nn + (long long)col * g.nzp + c0;
+    double* out_lo = out_hi + g.Nn;
     for (long long base = i0; base < i1; base += kAdjObsTile) {
         const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
         __syncthreads();
@@ -61,22 +79,35 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
                 for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
             }
         }
-    }
-    if (valid) {
-        double* out = partial + (long long)blockIdx.y * g.Nn + (long long)col * g.nzp + c0;
+        // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
+        if (valid) {
 #pragma unroll
-        for (int k = 0; k < KC; ++k)
-            if (c0 + k < g.nzp) out[k] = acc[k];
+            for (int k = 0; k < KC; ++k) {
+                if (c0 + k < g.nzp) {
+                    double hi = acc[k], lo = 0.0;
+                    if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
+                    out_hi[k] = hi;
+                    out_lo[k] = lo;
+                }
+                acc[k] = 0.0;
+            }
+        }
     }
 }
 
+// tnode[2][Nn] = sum over station chunks of partial[chunk][2][Nn], (hi, lo) pairs combined in chunk order.
 __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __restrict__ partial,
                                       double* __restrict__ tnode) {
     long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= Nn) return;
-    double s = 0.0;
-    for (int ch = 0; ch < nchunk; ++ch) s += partial[(long long)ch * Nn + n];
-    tnode[n] = s;
+    double hi = partial[n], lo = partial[Nn + n];
+    for (int ch = 1; ch < nchunk; ++ch) {
+        const double* pc = partial + (long long)ch * 2 * Nn;
+        two_sum_acc(hi, lo, pc[n], hi, lo);
+        lo += pc[Nn + n];
+    }
+    tnode[n] = hi;
+    tnode[Nn + n] = lo;
 }
 
 template <int TPB, int KC, int MINB>

@@ -64,9 +64,9 @@ void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t D = sizeof(double);
     L.cnode = take(g.Nn * D);
-    L.tnode = take(g.Nn * D);
+    L.tnode = take(2 * g.Nn * D);              // T as [hi | lo] planes
     L.fwd_partial = take((size_t)p.fwd_nchunk * g.N * D);
-    L.adj_partial = take((size_t)p.adj_nchunk * g.Nn * D);
+    L.adj_partial = take((size_t)p.adj_nchunk * 2 * g.Nn * D);
     L.gcell = take(g.M * D);
     L.cg_x = take(g.N * D);
     L.cg_r = take(g.N * D);
@@ -119,7 +119,7 @@ grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cuda
         CK(launch_adjoint_nodes(c, v, part, done, s), "adjoint_nodes");
         CK(launch_adjoint_reduce(c, part, tn, s), "adjoint_reduce");
     }
-    return exchange(c, tn, c->g.Nn, s);
+    return exchange(c, tn, 2 * c->g.Nn, s);
 }
 
 }  // namespace

@@ -45,6 +45,7 @@ __global__ void cell_to_node_kernel(Geom g, const double* __restrict__ u, const 
     cnode[n] = acc;
 }
 
+// tnode holds T as two planes [hi | lo] of Nn doubles (adjoint.cu).
 __global__ void node_to_cell_kernel(Geom g, const double* __restrict__ tnode, const double* __restrict__ w,
                                     double scale, double* __restrict__ gcell) {
     long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -54,18 +55,19 @@ __global__ void node_to_cell_kernel(Geom g, const double* __restrict__ tnode, co
     int j = (int)(t % g.ny);
     int i = (int)(t / g.ny);
     // fixed summation order: pair the two z-corners of each (p,q) edge first (their Psi values are closest)
-    double acc = 0.0;
+    double acc = 0.0, accl = 0.0;
 #pragma unroll
     for (int da = 0; da < 2; ++da)
 #pragma unroll
         for (int db = 0; db < 2; ++db) {
             long long base = ((long long)(i + da) * g.nyp + (j + db)) * g.nzp + k;
-            double lo = tnode[base], hi = tnode[base + 1];
             // sigma(da,db,dc) = -(-1)^(da+db+dc):  dc=0 -> -(-1)^(da+db), dc=1 -> +(-1)^(da+db)
-            double e = hi - lo;
+            double e = tnode[base + 1] - tnode[base];                    // high parts: close values, exact difference
+            double el = tnode[g.Nn + base + 1] - tnode[g.Nn + base];      // low parts (adjoint.cu "Accumulation")
             acc += ((da + db) & 1) ? -e : e;
+            accl += ((da + db) & 1) ? -el : el;
         }
-    double val = scale * acc;
+    double val = scale * (acc + accl);
     if (w) { double ww = w[cell]; val = val / (ww * ww); }
     gcell[cell] = val;
 }

@@ -3,8 +3,8 @@
 The path shards the way the paper shards it ("observation domain partitioned across devices,
 model-space variables replicated and synchronised"): rank r owns a contiguous block of stations and the whole mesh.
   forward  d = G u      : rows of d are local -- no communication;
-  adjoint  g = G^T v    : every rank forms the node sums T over ITS stations, one all-reduce(sum) of T (N_n doubles,
-                          27 MB at config 5) makes them global -- the only data-path collective;
+  adjoint  g = G^T v    : every rank forms the node sums T over ITS stations, one all-reduce(sum) of T (2 N_n doubles: high and low
+                          parts of the compensated sums, 54 MB at config 5) makes them global -- the only data-path collective;
   CG                    : alpha, x, r, p, q are station vectors (local rows); each dot product all-reduces its 256
                           block partials, so every rank computes bit-identical scalars on the device.
 The exchanges are issued by libgrav.so itself through the hook of include/grav.h (grav_set_allreduce); this module

@@ -84,13 +84,28 @@ def relmax(a, b, scale=None):
     return float(np.abs(np.asarray(a) - np.asarray(b)).max() / scale)
 
 
+def _gate(err, got_s, ref, truth_fn, scale, what):
+    """1e-10 of the global max against the FP64 oracle; where that fails, adjudicate against the long-double build
+    of the oracle (reading C15: the FP64 closed form has a cancellation floor of ~1e-10 of max for white-noise
+    inputs at config-4/5 scale): gpu_err <= max(1e-10, 2 x the FP64 oracle's own error)."""
+    if err <= TOL_OP:
+        print(f"{what}: gpu-vs-oracle {err:.2e}")
+        return
+    truth = truth_fn()
+    err_gpu, err_orc = relmax(got_s, truth, scale), relmax(ref, truth, scale)
+    print(f"{what}: gpu-vs-oracle {err:.2e}; vs long-double truth: gpu {err_gpu:.2e}, FP64 oracle {err_orc:.2e}")
+    assert err_gpu <= max(TOL_OP, 2.0 * err_orc), (what, err_gpu, err_orc)
+
+
 def test_forward_sampled_stations(case):
     wl, s = case.wl, case.sidx
-    for u in (wl.m_true, case.u_w):
+    for u, name in ((wl.m_true, "m_true"), (case.u_w, "white u")):
         got = host(case.ctx.forward(dev(u)))
         ref = oracle.forward(case.mesh, wl.xo[s], wl.yo[s], wl.zo[s], wl.gamma, u)
         assert np.all(np.isfinite(got))
-        assert relmax(got[s], ref, np.abs(got).max()) <= TOL_OP
+        scale = np.abs(got).max()
+        truth = lambda: oracle.forward(case.mesh, wl.xo[s], wl.yo[s], wl.zo[s], wl.gamma, u, prec=1)
+        _gate(relmax(got[s], ref, scale), got[s], ref, truth, scale, f"cfg{case.cfg} forward, {name}")
 
 
 def test_forward_whole_mesh_row_sums(case):
@@ -104,18 +119,13 @@ def test_forward_whole_mesh_row_sums(case):
 
 def test_adjoint_sampled_cells(case):
     wl, c = case.wl, case.cidx
-    for v, white in ((case.v_s, False), (case.v_w, True)):
+    for v, name in ((case.v_s, "smooth v"), (case.v_w, "white v")):
         got = host(case.ctx.adjoint(dev(v)))
         assert np.all(np.isfinite(got))
         scale = np.abs(got).max()
         ref = oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=c)
-        err = relmax(got[c], ref, scale)
-        if err > TOL_OP and white:
-            truth = oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=c, prec=1)
-            err_gpu, err_orc = relmax(got[c], truth, scale), relmax(ref, truth, scale)
-            assert err_gpu <= max(TOL_OP, 2.0 * err_orc), (err_gpu, err_orc)
-        else:
-            assert err <= TOL_OP, err
+        truth = lambda: oracle.adjoint(case.mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=c, prec=1)
+        _gate(relmax(got[c], ref, scale), got[c], ref, truth, scale, f"cfg{case.cfg} adjoint, {name}")
 
 
 def test_dot_product_full_size(case):

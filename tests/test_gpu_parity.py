@@ -300,10 +300,12 @@ def test_allreduce_hook_placement(cfg1):
         calls.clear()
         a = sh.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
         b = ref.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
-        assert relmax(host(a["alpha"]), host(b["alpha"])) <= 1e-10
-        assert np.abs(host(a["hist"]) / (np.sqrt(2.0) * host(b["hist"])) - 1).max() <= 1e-10
-        assert relmax(host(a["m"]), np.sqrt(2.0) * host(b["m"])) <= 1e-10
-        big = wl.n_nodes if mode == 0 else wl.M
+        # the two runs differ by rounding only (gamma*sqrt(2) is rounded), amplified over 8 CG iterations
+        # (~1e-9 at this depth); a missing or misplaced exchange changes the iterates at O(1)
+        assert relmax(host(a["alpha"]), host(b["alpha"])) <= 1e-7
+        assert np.abs(host(a["hist"]) / (np.sqrt(2.0) * host(b["hist"])) - 1).max() <= 1e-7
+        assert relmax(host(a["m"]), np.sqrt(2.0) * host(b["m"])) <= 1e-7
+        big = 2 * wl.n_nodes if mode == 0 else wl.M     # node sums travel as (hi, lo) planes
         # d.d, then per iteration: operator output, p.q, r.r; finally the model recovery
         assert calls == [256] + [big, 256, 256] * its + [big]
         # the adjoint is global (summed over the two ranks), the forward stays local
