@@ -30,9 +30,11 @@ UNIT = "pair evals/s"
 
 # FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
 # capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
-FP64_INST_PER_EVAL = {"forward_nodes": 48.0, "adjoint_nodes": 49.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture (profiles/)
-NCU_DRAM_BYTES = {"forward_nodes": None, "adjoint_nodes": None}
+FP64_INST_PER_EVAL = {"forward_nodes": 48.0, "adjoint_nodes": 48.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 5 from the committed `ncu --set full` capture
+# (profiles/r1_ncu_full_cfg5.md); None for other configs
+NCU_DRAM_BYTES = {5: {"forward_nodes": 31.7e6, "adjoint_nodes": 79.6e6}}
+NCU_DRAM_BYTES_STORED = {3: {"gemv": None, "gemvt": None}}
 FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
 
 
@@ -46,6 +48,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-stored", action="store_true", help="skip the stored-G (HBM-bound GEMV) measurement")
+    ap.add_argument("--stored-config", type=int, default=3, help="config whose G is tabulated for the stored-G leg")
     return ap.parse_args()
 
 
@@ -123,6 +127,68 @@ def cpu_oracle_rate(wl, seconds, sample_note=True):
     t, s = run(S)
     return dict(value=s * wl.M / t, unit=UNIT, cores=cores, kind="oracle",
                 sample=f"oracle.forward on {s} seeded stations x all {wl.M} prisms ({s * wl.M:.3g} pairs, {t:.1f} s)")
+
+
+
+def measured_hbm_peak():
+    """(GB/s, source): the driver-written copy bandwidth of this pool's B200s, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy read+write, burst)"
+    except Exception:
+        return 6500.0, "fallback (B200_PROFILING.md: ~6.5 TB/s measured copy bandwidth); MEASURED_PEAKS.json absent"
+
+
+def stored_g_leg(cfg, local, reps=5):
+    """BASELINE.json north_star kernel 4: tabulate G once (FP32 storage at config 3, reading C10), then time the
+    two HBM-bound mat-vecs d = G u and g = G^T v alone with CUDA events; algorithmic bytes = N*M*sizeof(elem)."""
+    import torch
+    from paper_2602_03857_b200 import binding, workloads
+    wl = workloads.make(cfg)
+    fp32 = wl.N * wl.M * 8 > 100e9
+    elem = 4 if fp32 else 8
+    dev = torch.device("cuda", local)
+    ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+    u = torch.as_tensor(np.ascontiguousarray(wl.m_true)).to(dev)
+    v = torch.as_tensor(np.random.default_rng(11).standard_normal(wl.N)).to(dev)
+    d = torch.empty(wl.N, dtype=torch.float64, device=dev)
+    g = torch.empty(wl.M, dtype=torch.float64, device=dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e0, e1 = ev(), ev()
+    l0 = ctx.launches
+    e0.record(); ctx.store_g(fp32=fp32); e1.record(); torch.cuda.synchronize()
+    t_tab = e0.elapsed_time(e1)
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):            # G (>= 4 GB) is far larger than the 126 MB L2: every pass streams from HBM
+            a, b = ev(), ev()
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts)
+
+    t_mv = timed(lambda: ctx.forward_stored(u, out=d))
+    t_mvt = timed(lambda: ctx.adjoint_stored(v, out=g))
+    launches = ctx.launches - l0
+    dm = ctx.forward(u)
+    err = float((d - dm).abs().max() / dm.abs().max())
+    nbytes = float(wl.N) * wl.M * elem
+    peak, src = measured_hbm_peak()
+    dom, t_dom = ("gemv", t_mv) if t_mv >= t_mvt else ("gemvt", t_mvt)
+    out = {"workload": wl.name, "elem": "f32" if fp32 else "f64", "g_bytes": nbytes,
+           "ms_tabulate": t_tab, "pairs_per_s_tabulate": float(wl.N) * wl.M / (t_tab * 1e-3),
+           "ms_gemv": t_mv, "ms_gemvt": t_mvt, "s_per_cg_iter_stored": (t_mv + t_mvt) * 1e-3,
+           "max_rel_err_vs_matrix_free_forward": err, "gpu_launches": launches,
+           "roofline": {"bound": "hbm", "kernel": dom, "achieved": nbytes / (t_dom * 1e-3) / 1e9, "peak": peak,
+                        "unit": "GB/s", "frac": nbytes / (t_dom * 1e-3) / 1e9 / peak,
+                        "traffic": NCU_DRAM_BYTES_STORED.get(cfg, {}).get(dom), "peak_source": src,
+                        "frac_of_8TBps_nominal": nbytes / (t_dom * 1e-3) / 1e9 / 8000.0,
+                        "gbs_gemv": nbytes / (t_mv * 1e-3) / 1e9, "gbs_gemvt": nbytes / (t_mvt * 1e-3) / 1e9}}
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -266,7 +332,7 @@ def run_ours(args):
     clk = (clocks or {}).get("sm_mhz") or 1965.0
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_nominal,
-        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": NCU_DRAM_BYTES.get(dom),
+        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": NCU_DRAM_BYTES.get(args.config, {}).get(dom),
         "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz = 1 DFMA/DMUL/DADD per lane per clock (DESIGN.md 6); "
                        f"DFMA-only probe in this run: {probe_rate / 1e12:.2f} T inst/s",
         "frac_of_probe": achieved / (probe_rate / 1e12),
@@ -301,6 +367,11 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_oracle_rate(wl, args.cpu_seconds)
 
+    stored = None
+    if rank == 0 and world == 1 and not args.no_stored:
+        sh.close()
+        stored = stored_g_leg(args.stored_config, local)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -314,6 +385,7 @@ def run_ours(args):
                        "l2": "flushed between steps (256 MiB write)", "lambda": lam,
                        "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "stored_g": stored,
         }
         print(json.dumps(line))
     sh.close()

@@ -160,6 +160,9 @@ grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
  * CPU-only tests can check it: returns Psi(X,Y,Z) + (X+Y)*k0*ln2 (the offset cancels in every signed sum, see
  * csrc/psi.cuh). */
 double grav_debug_psi_fast_host(double X, double Y, double Z, int k0);
+/* The same for the second-generation evaluator of csrc/psi2.cuh (swap-free atan2 reduction, exponent folded into
+ * the log table entry): returns Psi(X,Y,Z) + (X+Y)*k0*ln2. */
+double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0);
 /* The global exponent offset k0 chosen for this context (2^k0 ~ survey scale). */
 int grav_debug_k0(const grav_ctx* ctx);
 

@@ -21,7 +21,7 @@ EXPORTS = [
     "grav_forward", "grav_adjoint", "grav_depth_weights", "grav_dataspace_cg", "grav_store_g",
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_launch_count",
-    "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host",
+    "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host",
     "grav_debug_k0", "grav_debug_set_tuning", "grav_set_allreduce",
 ]
 
@@ -90,6 +90,8 @@ def load():
     L.grav_debug_set_psi_variant.argtypes = [vp, i]
     L.grav_debug_psi_fast_host.restype = d
     L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
+    L.grav_debug_psi2_fast_host.restype = d
+    L.grav_debug_psi2_fast_host.argtypes = [d, d, d, i]
     L.grav_debug_set_tuning.restype = i
     L.grav_debug_set_tuning.argtypes = [vp, i, i]
     L.grav_set_allreduce.restype = i
@@ -323,9 +325,10 @@ class GravContext:
         return int(self._lib.grav_launch_count(self._h))
 
 
-def psi_fast_host(X, Y, Z, k0=0):
-    """Host emulation of the device Psi evaluator (diagnostic; needs no GPU)."""
-    return float(load().grav_debug_psi_fast_host(float(X), float(Y), float(Z), int(k0)))
+def psi_fast_host(X, Y, Z, k0=0, gen=1):
+    """Host emulation of the device Psi evaluators (diagnostic; needs no GPU): gen 1 = psi.cuh, 2 = psi2.cuh."""
+    fn = load().grav_debug_psi2_fast_host if gen == 2 else load().grav_debug_psi_fast_host
+    return float(fn(float(X), float(Y), float(Z), int(k0)))
 
 
 def fp64_peak_probe(device=0, iters=200000):

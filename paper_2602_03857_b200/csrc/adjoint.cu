@@ -16,6 +16,7 @@
 // by adjoint_reduce with the same TwoSum.
 #include "grav_internal.cuh"
 #include "psi.cuh"
+#include "psi2.cuh"
 
 namespace grav {
 
@@ -30,15 +31,19 @@ __device__ __forceinline__ void two_sum_acc(double hi_in, double lo_in, double x
     lo_out = lo_in + err;
 }
 
-template <int TPB, int KC, int MINB, bool FAST>
-__global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
+// EV: 0 = CUDA libm (cross-check), 1 = psi_fast (psi.cuh), 2 = psi2_fast (psi2.cuh, the default)
+template <int TPB, int KC, int MINB, int EV>
+__global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, Psi2Dev pd2,
+                                                                        const double* __restrict__ v,
                                                                         double* __restrict__ partial, int ncg,
                                                                         int obs_per_chunk, const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
     PsiTabView tb;
-    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
+    Psi2TabView tb2;
+    if (EV == 1) tb = psi_tables_to_smem(s_tab, pd);
+    if (EV == 2) tb2 = psi2_tables_to_smem(s_tab, pd2);
     const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long nthreads = (long long)g.ncol * ncg;
     const bool valid = t < nthreads;
@@ -67,11 +72,12 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
         for (int j = 0; j < cnt; ++j) {
             const double4 o = s_obs[j];
             const double X = xa - o.x, Y = yb - o.y;
-            if (FAST) {
+            if (EV != 0) {
                 const PsiColumn pc = psi_column(X, Y);
                 const double vs = o.w * pc.s;
 #pragma unroll
-                for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_fast(tb, pc, zc[k] - o.z), acc[k]);
+                for (int k = 0; k < KC; ++k)
+                    acc[k] = fma(vs, EV == 1 ? psi_fast(tb, pc, zc[k] - o.z) : psi2_fast(tb2, pc, zc[k] - o.z), acc[k]);
             } else {
                 const double XY = X * Y;
                 const double Q = fma(Y, Y, X * X);
@@ -110,12 +116,13 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     tnode[Nn + n] = lo;
 }
 
-template <int TPB, int KC, int MINB>
+template <int TPB, int KC, int MINB, int EV = 1>
 static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
     static bool inited = false;
+    constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
     if (!inited) {
-        cudaError_t e = cudaFuncSetAttribute(adjoint_nodes_kernel<TPB, KC, MINB, true>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(adjoint_nodes_kernel<TPB, KC, MINB, EV>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         inited = true;
     }
@@ -123,8 +130,8 @@ static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial
     const int ncg = (c->g.nzp + KC - 1) / KC;
     const long long nthreads = (long long)c->g.ncol * ncg;
     dim3 grid((unsigned)((nthreads + TPB - 1) / TPB), p.adj_nchunk);
-    adjoint_nodes_kernel<TPB, KC, MINB, true><<<grid, TPB, kTabSmemBytes, s>>>(c->g, c->pd, v, partial, ncg,
-                                                                              p.adj_obs_per_chunk, done);
+    adjoint_nodes_kernel<TPB, KC, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, c->pd2, v, partial, ncg,
+                                                                    p.adj_obs_per_chunk, done);
     return cudaGetLastError();
 }
 
@@ -136,17 +143,33 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
     if (c->psi_variant == 0) {
         switch (c->tune[1]) {
             default:
-            case 0: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
+            case 0:   // the plan's choice of KC (grav_api.cu make_plan)
+                if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
+                else if (p.adj_kc == 6) e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s);
+                else e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s);
+                break;
+            case 12: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
             case 1: e = adj_launch_fast<256, 4, 3>(c, v, partial, done, s); break;
             case 2: e = adj_launch_fast<256, 8, 2>(c, v, partial, done, s); break;
             case 3: e = adj_launch_fast<128, 8, 4>(c, v, partial, done, s); break;
             case 4: e = adj_launch_fast<256, 2, 3>(c, v, partial, done, s); break;
             case 5: e = adj_launch_fast<256, 4, 2>(c, v, partial, done, s); break;
             case 6: e = adj_launch_fast<256, 2, 4>(c, v, partial, done, s); break;
+            case 7: e = adj_launch_fast<128, 8, 2>(c, v, partial, done, s); break;
+            case 8: e = adj_launch_fast<128, 8, 3>(c, v, partial, done, s); break;
+            case 9: e = adj_launch_fast<128, 6, 3>(c, v, partial, done, s); break;
+            case 10: e = adj_launch_fast<128, 4, 3>(c, v, partial, done, s); break;
+            case 11: e = adj_launch_fast<128, 16, 2>(c, v, partial, done, s); break;
+            case 21: e = adj_launch_fast<128, 4, 3, 2>(c, v, partial, done, s); break;
+            case 23: e = adj_launch_fast<128, 8, 3, 2>(c, v, partial, done, s); break;
+            case 24: e = adj_launch_fast<256, 6, 1, 2>(c, v, partial, done, s); break;
+            case 25: e = adj_launch_fast<256, 8, 1, 2>(c, v, partial, done, s); break;
+            case 26: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
         }
     } else {
-        dim3 grid(p.adj_blocks, p.adj_nchunk);
-        adjoint_nodes_kernel<128, 4, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, v, partial, p.adj_ncg,
+        const int ncg4 = (c->g.nzp + 3) / 4;
+        dim3 grid((unsigned)(((long long)c->g.ncol * ncg4 + 127) / 128), p.adj_nchunk);
+        adjoint_nodes_kernel<128, 4, 4, 0><<<grid, 128, 0, s>>>(c->g, c->pd, c->pd2, v, partial, ncg4,
                                                                     p.adj_obs_per_chunk, done);
         e = cudaGetLastError();
     }

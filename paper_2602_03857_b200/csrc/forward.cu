@@ -9,17 +9,22 @@
 // Bound: FP64 pipe: ~49 FP64 instructions per evaluation, 8 bytes of c_n per warp.
 #include "grav_internal.cuh"
 #include "psi.cuh"
+#include "psi2.cuh"
 
 namespace grav {
 
-template <int TPB, int UNROLL, int MINB, bool FAST>
-__global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ cnode,
+// EV: 0 = CUDA libm (cross-check), 1 = psi_fast (psi.cuh), 2 = psi2_fast (psi2.cuh, the default)
+template <int TPB, int UNROLL, int MINB, int EV>
+__global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, Psi2Dev pd2,
+                                                                        const double2* __restrict__ cnode,
                                                                         double* __restrict__ partial, int cols_per_chunk,
                                                                         const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     PsiTabView tb;
-    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
+    Psi2TabView tb2;
+    if (EV == 1) tb = psi_tables_to_smem(s_tab, pd);
+    if (EV == 2) tb2 = psi2_tables_to_smem(s_tab, pd2);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
@@ -30,23 +35,25 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
     double X = __ldg(g.xn + a) - xo;
     for (int col = col0; col < col1; ++col) {
         const double Y = __ldg(g.yn + b) - yo;
-        const double* __restrict__ cc = cnode + (long long)col * g.nzp;
+        const double2* __restrict__ cc = cnode + (long long)col * g.nzp;   // (c_n, zn[c]) pairs: one LDG.128
         double colacc = 0.0;
-        if (FAST) {
+        if (EV != 0) {
             const PsiColumn pc = psi_column(X, Y);
 #pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
-                const double Z = __ldg(g.zn + c) - zo;
-                const double coef = __ldg(cc + c);
-                colacc = fma(coef, psi_fast(tb, pc, Z), colacc);
+                const double2 cz = __ldg(cc + c);
+                const double Z = cz.y - zo;
+                const double coef = cz.x;
+                colacc = fma(coef, EV == 1 ? psi_fast(tb, pc, Z) : psi2_fast(tb2, pc, Z), colacc);
             }
             colacc *= pc.s;
         } else {
             const double XY = X * Y;
             const double Q = fma(Y, Y, X * X);
             for (int c = 0; c < g.nzp; ++c) {
-                const double Z = __ldg(g.zn + c) - zo;
-                const double coef = __ldg(cc + c);
+                const double2 cz = __ldg(cc + c);
+                const double Z = cz.y - zo;
+                const double coef = cz.x;
                 colacc = fma(coef, psi_libm(X, Y, Z, XY, Q), colacc);
             }
         }
@@ -92,41 +99,55 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
 }
 
 // Launch variants (grav_debug_set_tuning(ctx, 0, v)); the default is the one measured fastest (profiles/).
-template <int TPB, int UNROLL, int MINB>
-static cudaError_t fwd_launch_fast(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
+template <int TPB, int UNROLL, int MINB, int EV = 1>
+static cudaError_t fwd_launch_fast(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
     static bool inited = false;
+    constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
     if (!inited) {
-        cudaError_t e = cudaFuncSetAttribute(forward_nodes_kernel<TPB, UNROLL, MINB, true>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(forward_nodes_kernel<TPB, UNROLL, MINB, EV>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         inited = true;
     }
     const Plan& p = c->plan;
     dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);
-    forward_nodes_kernel<TPB, UNROLL, MINB, true><<<grid, TPB, kTabSmemBytes, s>>>(c->g, c->pd, cnode, partial,
-                                                                                  p.fwd_cols_per_chunk, done);
+    forward_nodes_kernel<TPB, UNROLL, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, c->pd2, cnode, partial,
+                                                                        p.fwd_cols_per_chunk, done);
     return cudaGetLastError();
 }
 
 cudaError_t init_forward_kernels() { return cudaSuccess; }
 
-cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s) {
+cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* partial, const int* done, cudaStream_t s) {
     const Plan& p = c->plan;
+    const double2* cnode = reinterpret_cast<const double2*>(cnode_);
     cudaError_t e;
     if (c->psi_variant == 0) {
         switch (c->tune[0]) {
             default:
-            case 0: e = fwd_launch_fast<128, 2, 4>(c, cnode, partial, done, s); break;
+            case 0: e = fwd_launch_fast<256, 4, 2, 2>(c, cnode, partial, done, s); break;
+            case 12: e = fwd_launch_fast<128, 2, 4>(c, cnode, partial, done, s); break;
             case 1: e = fwd_launch_fast<256, 1, 3>(c, cnode, partial, done, s); break;
             case 2: e = fwd_launch_fast<256, 2, 2>(c, cnode, partial, done, s); break;
             case 3: e = fwd_launch_fast<128, 1, 4>(c, cnode, partial, done, s); break;
             case 4: e = fwd_launch_fast<256, 1, 4>(c, cnode, partial, done, s); break;
             case 5: e = fwd_launch_fast<256, 4, 2>(c, cnode, partial, done, s); break;
             case 6: e = fwd_launch_fast<512, 2, 1>(c, cnode, partial, done, s); break;
+            case 7: e = fwd_launch_fast<128, 4, 3>(c, cnode, partial, done, s); break;
+            case 8: e = fwd_launch_fast<128, 4, 2>(c, cnode, partial, done, s); break;
+            case 9: e = fwd_launch_fast<128, 3, 3>(c, cnode, partial, done, s); break;
+            case 10: e = fwd_launch_fast<128, 2, 3>(c, cnode, partial, done, s); break;
+            case 11: e = fwd_launch_fast<128, 8, 2>(c, cnode, partial, done, s); break;
+            case 20: e = fwd_launch_fast<256, 2, 2, 2>(c, cnode, partial, done, s); break;
+            case 22: e = fwd_launch_fast<128, 2, 3, 2>(c, cnode, partial, done, s); break;
+            case 23: e = fwd_launch_fast<128, 4, 3, 2>(c, cnode, partial, done, s); break;
+            case 24: e = fwd_launch_fast<256, 1, 3, 2>(c, cnode, partial, done, s); break;
+            case 25: e = fwd_launch_fast<512, 2, 1, 2>(c, cnode, partial, done, s); break;
+            case 26: e = fwd_launch_fast<256, 3, 2, 2>(c, cnode, partial, done, s); break;
         }
     } else {
-        dim3 grid(p.fwd_tiles, p.fwd_nchunk);
-        forward_nodes_kernel<128, 1, 4, false><<<grid, 128, 0, s>>>(c->g, c->pd, cnode, partial, p.fwd_cols_per_chunk, done);
+        dim3 grid((unsigned)((c->g.N + 127) / 128), p.fwd_nchunk);
+        forward_nodes_kernel<128, 1, 4, 0><<<grid, 128, 0, s>>>(c->g, c->pd, c->pd2, cnode, partial, p.fwd_cols_per_chunk, done);
         e = cudaGetLastError();
     }
     c->launches++;

@@ -34,23 +34,36 @@ int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Launch plan: enough blocks to fill 148 SMs several times over, fixed per context => deterministic sums.
 void make_plan(const Geom& g, Plan& p) {
-    const int target_blocks = 148 * 16;
-    // forward: 128 stations per block; split the node columns into chunks when the station tiles are few
-    p.fwd_tpb = 128;
+    // Blocks of one launch all take the same time, so a grid of W.f waves of resident blocks costs ceil(W.f) waves:
+    // with ~5 waves (the first plan) up to 18 % of the launch was tail.  ~100 blocks per SM keeps the tail <= 2-3 %
+    // (profiles/r1_tail_and_variants.md); the price is a larger partial buffer (<= 40 MB), read once.
+    const int target_blocks = 148 * 96;
+    // forward: 256 stations per block; split the node columns into chunks when the station tiles are few
+    p.fwd_tpb = 256;
     p.fwd_obs_per_thread = 1;
     p.fwd_tiles = ceil_div(g.N, p.fwd_tpb * p.fwd_obs_per_thread);
     int want = ceil_div(target_blocks, p.fwd_tiles);
     if (want > g.ncol) want = g.ncol;
     if (want > 1024) want = 1024;
+    while (want > 1 && (double)want * g.N * 8.0 > 64e6) --want;      // partial buffer <= 64 MB
     if (want < 1) want = 1;
     p.fwd_cols_per_chunk = ceil_div(g.ncol, want);
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
-    p.adj_tpb = 128;
+    // KC nodes per thread: per-(thread, station) set-up (~22 issue cycles) is shared by KC evaluations (~115 each)
+    // but the column is padded to a multiple of KC; pick the cheapest of the compiled variants for this nz.
+    p.adj_tpb = 256;
     p.adj_kc = 4;
+    double best = 1e300;
+    for (int kc = 4; kc <= 6; ++kc) {
+        const double cost = (115.0 + 22.0 / kc) * (double)(ceil_div(g.nzp, kc) * kc);
+        if (cost < best) { best = cost; p.adj_kc = kc; }
+    }
+    if (p.adj_kc == 6) p.adj_tpb = 128;
     p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
-    want = ceil_div(target_blocks, p.adj_blocks);
+    want = ceil_div(148 * 128, p.adj_blocks);
+    while (want > 1 && (double)want * 2.0 * g.Nn * 8.0 > 256e6) --want;   // [hi|lo] partial planes <= 256 MB
     int maxchunk = ceil_div(g.N, 64);
     if (want > maxchunk) want = maxchunk;
     if (want > 256) want = 256;
@@ -63,7 +76,7 @@ void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t D = sizeof(double);
-    L.cnode = take(g.Nn * D);
+    L.cnode = take(2 * g.Nn * D);              // (c_n, zn[c]) pairs
     L.tnode = take(2 * g.Nn * D);              // T as [hi | lo] planes
     L.fwd_partial = take((size_t)p.fwd_nchunk * g.N * D);
     L.adj_partial = take((size_t)p.adj_nchunk * 2 * g.Nn * D);
@@ -167,7 +180,8 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     c->device = device;
 
     const size_t ntab = sizeof(PsiTablesHost) / sizeof(double);
-    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + 7 * 32;   // each array 256-byte aligned
+    const size_t ntab2 = sizeof(Psi2TablesHost) / sizeof(double);
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2 + 8 * 32;   // each array 256-byte aligned
     std::vector<double> host;
     try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
     void* dev = nullptr;
@@ -196,6 +210,10 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         if (c->pd.k0 > 900) c->pd.k0 = 900;
         if (c->pd.k0 < -900) c->pd.k0 = -900;
         c->pd.k = psi_consts_make(c->pd.k0);
+        static Psi2TablesHost tabs2;      // ~8 KB; regenerated per context (depends on k0)
+        psi2_tables_generate(&tabs2, c->pd.k0);
+        c->pd2.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs2), ntab2));
+        c->pd2.k = psi2_consts_make(c->pd.k0);
         c->psi_variant = 0;
     }
     e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
@@ -274,6 +292,15 @@ double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
     tb.base = tabs.e; tb.shift = 0; tb.k = psi_consts_make(k0); tb.ik = psi_int_consts(0);
     const PsiColumn pc = psi_column(X, Y);
     return pc.s * psi_fast(tb, pc, Z);
+}
+
+double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0) {
+    Psi2TablesHost tabs;
+    psi2_tables_generate(&tabs, k0);
+    Psi2TabView tb;
+    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0);
+    const PsiColumn pc = psi_column(X, Y);
+    return pc.s * psi2_fast(tb, pc, Z);
 }
 
 grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {

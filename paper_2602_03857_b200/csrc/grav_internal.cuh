@@ -6,6 +6,7 @@
 
 #include "../../include/grav.h"
 #include "psi.cuh"
+#include "psi2.cuh"
 
 namespace grav {
 
@@ -61,6 +62,7 @@ struct grav_ctx {
     size_t ws_bytes;
     int stored_elem;         // 0 none, 8 FP64, 4 FP32
     grav::PsiDev pd;         // Psi tables (inside geom_dev) and the global exponent offset k0
+    grav::Psi2Dev pd2;       // tables and constants of the second-generation evaluator (psi2.cuh), same k0
     int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
     int tune[4];             // launch-variant selectors (grav_debug_set_tuning): 0 forward, 1 adjoint
     grav_allreduce_fn allreduce;   // observation-sharded operation: sum over ranks (NULL = single rank)

@@ -42,7 +42,8 @@ __global__ void cell_to_node_kernel(Geom g, const double* __restrict__ u, const 
             }
         }
     }
-    cnode[n] = acc;
+    // stored with the node depth beside it, so that the forward z-loop needs ONE 16-byte load per evaluation
+    reinterpret_cast<double2*>(cnode)[n] = make_double2(acc, g.zn[c]);
 }
 
 // tnode holds T as two planes [hi | lo] of Nn doubles (adjoint.cu).

@@ -11,8 +11,18 @@ from paper_2602_03857_b200 import binding
 LN2 = math.log(2.0)
 
 
+GEN = 1      # evaluator generation under test (set by the autouse fixture: every test runs for psi.cuh and psi2.cuh)
+
+
+@pytest.fixture(autouse=True, params=[1, 2], ids=["psi", "psi2"])
+def _generation(request):
+    global GEN
+    GEN = request.param
+    yield
+
+
 def _scaled_err(X, Y, Z, k0=0):
-    got = binding.psi_fast_host(X, Y, Z, k0) - (X + Y) * k0 * LN2
+    got = binding.psi_fast_host(X, Y, Z, k0, GEN) - (X + Y) * k0 * LN2
     ref = oracle.psi(X, Y, Z, 1)
     R = math.sqrt(X * X + Y * Y + Z * Z)
     if R == 0:
@@ -38,7 +48,7 @@ def test_psi_fast_random(scale):
 def test_psi_fast_guards_and_special_points():
     for args in [(0, 0, 0), (0, -5, 0), (2, 3, 0), (0, 0, 5), (1, 1, 1), (3, -4, 0), (-3, 4, 1e-9), (0, 5, 2),
                  (5, 0, 2), (-5, 0, -2), (1e-8, -1e4, 1e-8), (7, 7, 7), (7, -7, -7)]:
-        got = binding.psi_fast_host(*args, 0)
+        got = binding.psi_fast_host(*args, 0, GEN)
         assert math.isfinite(got)
         ref = oracle.psi(*args, 1)
         assert abs(got - ref) <= 1e-15 * max(1.0, abs(ref)) + 1e-12 * (args == (1e-8, -1e4, 1e-8))
