@@ -30,11 +30,11 @@ UNIT = "pair evals/s"
 
 # FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
 # capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
-FP64_INST_PER_EVAL = {"forward_nodes": 48.0, "adjoint_nodes": 48.0}
+FP64_INST_PER_EVAL = {"forward_nodes": 46.0, "adjoint_nodes": 46.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 5 from the committed `ncu --set full` capture
 # (profiles/r1_ncu_full_cfg5.md); None for other configs
-NCU_DRAM_BYTES = {5: {"forward_nodes": 31.7e6, "adjoint_nodes": 79.6e6}}
-NCU_DRAM_BYTES_STORED = {3: {"gemv": None, "gemvt": None}}
+NCU_DRAM_BYTES = {5: {"forward_nodes": 76.6e6, "adjoint_nodes": 453.1e6}}
+NCU_DRAM_BYTES_STORED = {3: {"gemv": 68.745e9, "gemvt": None}}      # profiles/r1_ncu_full_gemv_cfg3.md
 FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
 
 
@@ -48,6 +48,12 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--probe", action="store_true",
+                    help="print the FP64 issue microbenchmark table (grav_fp64_mix_probe) and exit")
+    ap.add_argument("--no-paper-shape", action="store_true",
+                    help="skip the paper-shaped run (Table 1 shape: Float32 G build + outer inversion loop)")
+    ap.add_argument("--paper-shape-matrix-free", action="store_true",
+                    help="also run the outer inversion loop matrix-free in FP64 on the paper's shape (~1 min)")
     ap.add_argument("--no-stored", action="store_true", help="skip the stored-G (HBM-bound GEMV) measurement")
     ap.add_argument("--stored-config", type=int, default=3, help="config whose G is tabulated for the stored-G leg")
     return ap.parse_args()
@@ -189,6 +195,50 @@ def stored_g_leg(cfg, local, reps=5):
     del ctx
     torch.cuda.empty_cache()
     return out
+
+
+def paper_shape_leg(local, matrix_free=False):
+    """the paper's own pipeline on the SHAPE of its largest single-GPU benchmark (Table 1,
+    P:168-178: 2,601 stations x 3.28e6 cells, Float32 G = 34.1 GB): build G in Float32, then the outer model-update
+    loop (<= 30 updates x <= 20 CG iterations, tolerances 1e-4) with the stored G.  Wall clock around the
+    synchronising C-ABI calls.  The paper's 63.88 s (1x A100 40 GB) / 1007.46 s (EPYC 7H12) are quoted as context:
+    different hardware, different (unavailable) model and data."""
+    import torch
+    from paper_2602_03857_b200 import binding, workloads
+    wl = workloads.make(6)
+    dev = torch.device("cuda", local)
+    ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+    w = ctx.depth_weights(wl.beta, wl.z0)
+    d_clean = ctx.forward(torch.as_tensor(np.ascontiguousarray(wl.m_true)).to(dev))
+    d_obs = d_clean + wl.noise_frac * float(d_clean.abs().max()) * torch.as_tensor(wl.noise()).to(dev)
+    lam = wl.lam_factor * float(ctx.gram_diag(w).mean().item())
+    ctx.set_mode(binding.STORED_F32)
+    torch.cuda.synchronize()
+    l0 = ctx.launches
+    t0 = time.perf_counter()
+    ctx.store_g(fp32=True)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    out = ctx.invert(d_obs, w, lam, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4,
+                     mode=binding.STORED_F32)
+    torch.cuda.synchronize()
+    t2 = time.perf_counter()
+    res = {"workload": wl.name, "prisms": wl.M, "stations": wl.N, "g_bytes_f32": float(wl.N) * wl.M * 4,
+           "build_s": t1 - t0, "inversion_s": t2 - t1, "total_s": t2 - t0, "outer_updates": out["n_outer"],
+           "rel_residual": float(out["hist"][-1]), "gpu_launches": ctx.launches - l0, "lambda": lam,
+           "paper_context": {"total_s_1xA100_f32": 63.88, "total_s_cpu_epyc7h12": 1007.46,
+                             "source": "PAPER.md Table 1 (P:168-178), 3.28e6 cells x 2,601 stations"}}
+    if matrix_free:
+        t3 = time.perf_counter()
+        out2 = ctx.invert(d_obs, w, lam, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4)
+        torch.cuda.synchronize()
+        res["matrix_free_f64_total_s"] = time.perf_counter() - t3
+        res["matrix_free_f64_outer_updates"] = out2["n_outer"]
+        res["model_diff_f32_vs_f64"] = float((out["m"] - out2["m"]).abs().max() / out2["m"].abs().max())
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    return res
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -372,6 +422,11 @@ def run_ours(args):
         sh.close()
         stored = stored_g_leg(args.stored_config, local)
 
+    paper = None
+    if rank == 0 and world == 1 and not args.no_paper_shape:
+        sh.close()
+        paper = paper_shape_leg(local, args.paper_shape_matrix_free)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -385,7 +440,7 @@ def run_ours(args):
                        "l2": "flushed between steps (256 MiB write)", "lambda": lam,
                        "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "stored_g": stored,
+            "stored_g": stored, "paper_shape": paper,
         }
         print(json.dumps(line))
     sh.close()
@@ -393,8 +448,26 @@ def run_ours(args):
         torch.distributed.destroy_process_group()
 
 
+def run_probe():
+    """FP64 pipe utilisation of K DFMA chains per warp interleaved with NI integer instructions, W warps per
+    scheduler (include/grav.h: grav_fp64_mix_probe).  One JSON line per case."""
+    import torch
+    from paper_2602_03857_b200 import binding
+    assert torch.cuda.is_available()
+    clk = 1.965e9
+    for W in (1, 2, 4, 8, 16):
+        for K, NI in ((1, 0), (2, 0), (4, 0), (8, 0), (2, 1), (2, 2), (4, 1), (4, 2), (4, 4), (8, 2), (8, 4), (8, 8)):
+            n, ms = binding.fp64_mix_probe(0, K, NI, W, 20000 // K)
+            cyc = ms * 1e-3 * clk
+            print(json.dumps({"warps_per_scheduler": W, "dfma_chains": K, "int_per_group": NI,
+                              "int_per_dfma": NI / K, "fp64_pipe_util": round(2 * n / cyc, 4),
+                              "cycles_per_dfma": round(cyc / n, 3), "assumed_sm_hz": clk}))
+
+
 def main():
     args = parse()
+    if args.probe:
+        return run_probe()
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -122,6 +122,24 @@ grav_status grav_gram_diag(grav_ctx* ctx, const double* w_dev, double* diag_dev,
 grav_status grav_direct_solve(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda,
                               double* A_dev, double* alpha_dev, double* m_dev, void* stream);
 
+/* The paper's outer model-update loop around the data-space CG (<= 30 outer updates, <= 20 inner CG
+ * iterations, both stopped at res <= 1e-4; "Gauss-Newton-style update loop with step-size backtracking";
+ * Eq. 10-11, for the update itself).  The paper prints neither the residual norm nor the backtracking
+ * rule; DESIGN.md 2 (R1-R4) fixes them, and parity with the PAPER's loop is therefore unpinned (the oracle restates
+ * the same readings):
+ *   m_0 = m_ref (NULL = 0);  r_k = d_obs - G m_k;  stop when ||r_k||_2 / ||d_obs||_2 <= tol_outer or k = max_outer;
+ *   alpha = CG on (G W^-2 G^T + lambda I) alpha = r_k, <= max_inner iterations, stopped at ||res|| <= tol_inner ||r_k||;
+ *   delta_m = W^-2 G^T alpha;  s = 1, halved at most 10 times until ||r_k - s G delta_m|| < ||r_k||
+ *   (no decrease: stop with m_k);  m_{k+1} = m_k + s delta_m.
+ * dobs_dev[N], w_dev[M], mref_dev[M] or NULL, m_dev[M] out, dpred_dev[N] out or NULL (= G m): DEVICE.
+ * hist_host[max_outer + 1] (||r_k|| / ||d_obs||, entries 0..*n_outer_host), step_host[max_outer] (accepted s per
+ * update, 0 = rejected), n_outer_host (updates applied): HOST, each may be NULL.  mode as in grav_dataspace_cg.
+ * SYNCHRONISES the stream once per trial step (one scalar read back); needs the workspace. */
+grav_status grav_invert(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda,
+                        const double* mref_dev, int max_outer, int max_inner, double tol_outer, double tol_inner,
+                        int mode, double* m_dev, double* dpred_dev, double* hist_host, double* step_host,
+                        int* n_outer_host, void* stream);
+
 /* End-to-end variants with HOST buffers: host->device copy of the inputs, the same kernels, device->host copy
  * of the result, then cudaStreamSynchronize(stream).  Staging buffers live in the workspace. */
 grav_status grav_forward_host(grav_ctx* ctx, const double* u_host, double* d_host, void* stream);
@@ -148,6 +166,14 @@ long long grav_launch_count(const grav_ctx* ctx);
  * returns the number of FP64 thread-instructions executed in *ninstr and the elapsed ms in *ms (synchronises).
  * Used to confirm the FP64 pipe peak in the same run as the roofline numbers. */
 grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* ms);
+/* FP64 issue microbenchmark (csrc/probe.cu): every warp runs `chains` independent dependent-DFMA chains with `others`
+ * integer instructions after each group of `chains` DFMAs, `warps_per_smsp` (1..16) warps per scheduler on every SM.
+ * Supported (chains, others): (1|2|4|8, 0), (2, 1|2), (4, 1|2|4), (8, 2|4|8); anything else returns GRAV_EINVAL.
+ * Returns the DFMA warp-instructions one scheduler executed and the elapsed ms (synchronises): the FP64 pipe
+ * accepts one warp-instruction per 2 cycles per scheduler, so utilisation = 2 * n / (ms * 1e-3 * sm_clock_hz).
+ * Diagnostic only; holds none of the method's arithmetic. */
+grav_status grav_fp64_mix_probe(int device, int chains, int others, int warps_per_smsp, int iters,
+                                double* dfma_warp_inst_per_smsp, double* ms);
 
 /* Diagnostics.  variant 0 (default): hand-built Psi evaluator (table-driven ln, reduced-argument atan, MUFU-seeded
  * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same kernels with CUDA libm (sqrt, /, atan, log).  Both are

@@ -20,8 +20,8 @@ EXPORTS = [
     "grav_mesh_create", "grav_mesh_destroy", "grav_sizes", "grav_workspace_bytes", "grav_set_workspace",
     "grav_forward", "grav_adjoint", "grav_depth_weights", "grav_dataspace_cg", "grav_store_g",
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
-    "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_launch_count",
-    "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host",
+    "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
+    "grav_fp64_peak_probe", "grav_fp64_mix_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host",
     "grav_debug_k0", "grav_debug_set_tuning", "grav_set_allreduce",
 ]
 
@@ -86,6 +86,10 @@ def load():
     L.grav_launch_count.argtypes = [vp]
     L.grav_fp64_peak_probe.restype = i
     L.grav_fp64_peak_probe.argtypes = [i, i, dp, dp]
+    L.grav_invert.restype = i
+    L.grav_invert.argtypes = [vp, vp, vp, d, vp, i, i, d, d, i, vp, vp, vp, vp, C.POINTER(C.c_int), vp]
+    L.grav_fp64_mix_probe.restype = i
+    L.grav_fp64_mix_probe.argtypes = [i, i, i, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.grav_debug_set_psi_variant.restype = i
     L.grav_debug_set_psi_variant.argtypes = [vp, i]
     L.grav_debug_psi_fast_host.restype = d
@@ -230,6 +234,23 @@ class GravContext:
                                            C.c_void_p(hist.data_ptr()), C.c_void_p(ab.data_ptr()), _stream()))
         return dict(alpha=alpha, m=m, hist=hist, ab=ab[:2 * iters].view(-1, 2) if iters else ab[:0])
 
+    def invert(self, dobs, w, lam, mref=None, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4,
+               mode=MATRIX_FREE, want_dpred=True):
+        """The paper's outer model-update loop (include/grav.h: grav_invert).  Returns dict(m, dpred, hist, steps,
+        n_outer); hist / steps are numpy arrays."""
+        m = self._new(self.M)
+        dpred = self._new(self.N) if want_dpred else None
+        hist = np.zeros(max_outer + 1)
+        steps = np.zeros(max(max_outer, 1))
+        n_outer = C.c_int(0)
+        _check(self._lib.grav_invert(self._h, _dev(dobs, self.N, "dobs"), _dev(w, self.M, "w"), float(lam),
+                                     _dev(mref, self.M, "mref"), int(max_outer), int(max_inner), float(tol_outer),
+                                     float(tol_inner), int(mode), _dev(m, self.M, "m"), _dev(dpred, self.N, "dpred"),
+                                     C.c_void_p(hist.ctypes.data), C.c_void_p(steps.ctypes.data), C.byref(n_outer),
+                                     _stream()))
+        k = n_outer.value
+        return dict(m=m, dpred=dpred, hist=hist[:k + 1], steps=steps[:k], n_outer=k)
+
     def store_g(self, fp32=False):
         want = STORED_F32 if fp32 else STORED_F64
         need = int(self._lib.grav_workspace_bytes(self._h, want))
@@ -336,3 +357,10 @@ def fp64_peak_probe(device=0, iters=200000):
     n, ms = C.c_double(), C.c_double()
     _check(load().grav_fp64_peak_probe(device, iters, C.byref(n), C.byref(ms)))
     return n.value / (ms.value * 1e-3), ms.value
+
+
+def fp64_mix_probe(device, chains, others, warps_per_smsp, iters=20000):
+    """(DFMA warp-instructions per scheduler, ms) of the FP64 issue microbenchmark (include/grav.h)."""
+    n, ms = C.c_double(), C.c_double()
+    _check(load().grav_fp64_mix_probe(device, chains, others, warps_per_smsp, iters, C.byref(n), C.byref(ms)))
+    return n.value, ms.value

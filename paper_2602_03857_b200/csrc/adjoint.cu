@@ -141,30 +141,18 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
     const Plan& p = c->plan;
     cudaError_t e;
     if (c->psi_variant == 0) {
-        switch (c->tune[1]) {
+        switch (c->tune[1]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
             default:
-            case 0:   // the plan's choice of KC (grav_api.cu make_plan)
+            case 0:   // shipped: the plan's choice of KC (grav_api.cu make_plan)
                 if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
                 else if (p.adj_kc == 6) e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s);
                 else e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s);
                 break;
-            case 12: e = adj_launch_fast<128, 4, 4>(c, v, partial, done, s); break;
-            case 1: e = adj_launch_fast<256, 4, 3>(c, v, partial, done, s); break;
-            case 2: e = adj_launch_fast<256, 8, 2>(c, v, partial, done, s); break;
-            case 3: e = adj_launch_fast<128, 8, 4>(c, v, partial, done, s); break;
-            case 4: e = adj_launch_fast<256, 2, 3>(c, v, partial, done, s); break;
-            case 5: e = adj_launch_fast<256, 4, 2>(c, v, partial, done, s); break;
-            case 6: e = adj_launch_fast<256, 2, 4>(c, v, partial, done, s); break;
-            case 7: e = adj_launch_fast<128, 8, 2>(c, v, partial, done, s); break;
-            case 8: e = adj_launch_fast<128, 8, 3>(c, v, partial, done, s); break;
-            case 9: e = adj_launch_fast<128, 6, 3>(c, v, partial, done, s); break;
-            case 10: e = adj_launch_fast<128, 4, 3>(c, v, partial, done, s); break;
-            case 11: e = adj_launch_fast<128, 16, 2>(c, v, partial, done, s); break;
-            case 21: e = adj_launch_fast<128, 4, 3, 2>(c, v, partial, done, s); break;
-            case 23: e = adj_launch_fast<128, 8, 3, 2>(c, v, partial, done, s); break;
-            case 24: e = adj_launch_fast<256, 6, 1, 2>(c, v, partial, done, s); break;
-            case 25: e = adj_launch_fast<256, 8, 1, 2>(c, v, partial, done, s); break;
-            case 26: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
+            case 1: e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s); break;
+            case 2: e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s); break;
+            case 3: e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s); break;
+            case 4: e = adj_launch_fast<128, 4, 4, 1>(c, v, partial, done, s); break;          // first generation
+            case 5: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
         }
     } else {
         const int ncg4 = (c->g.nzp + 3) / 4;

@@ -91,6 +91,11 @@ void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
     L.stage_m = take(g.M * D);
     L.stage_n = take(g.N * D);
     L.stage_hist = take(4096 * D);
+    L.inv_dm = take(g.M * D);
+    L.inv_r = take(g.N * D);
+    L.inv_dd = take(g.N * D);
+    L.inv_try = take(g.N * D);
+    L.inv_scal = take(8 * D);
     L.matfree_end = off;
     L.gemvt_partial = take((size_t)gemvt_chunks(g.N) * g.M * D);
     L.gstore = off;
@@ -476,6 +481,80 @@ grav_status grav_direct_solve(grav_ctx* c, const double* dobs, const double* w, 
     CK(launch_form_A(c, G, w, lambda, A, s), "form_A");
     CK(launch_cholesky_solve(c, A, dobs, alpha, (int)c->g.N, s), "cholesky_solve");
     if (m) CK(launch_gemvt(c, G, 8, alpha, w, m, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
+    return GRAV_OK;
+}
+
+// ---- outer model-update loop (csrc/invert.cu has the passage and the readings) -----------------------------
+grav_status grav_invert(grav_ctx* c, const double* dobs, const double* w, double lambda, const double* mref,
+                        int max_outer, int max_inner, double tol_outer, double tol_inner, int mode, double* m,
+                        double* dpred, double* hist_host, double* step_host, int* n_outer_host, void* stream) {
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!dobs || !w || !m) return fail(GRAV_EINVAL, "NULL vector");
+    if (max_outer < 0 || max_inner < 1 || !(tol_outer >= 0.0) || !(tol_inner >= 0.0) || !(lambda == lambda))
+        return fail(GRAV_EINVAL, "bad max_outer / max_inner / tolerance / lambda");
+    if (mode != GRAV_MATRIX_FREE && mode != GRAV_STORED_F64 && mode != GRAV_STORED_F32)
+        return fail(GRAV_EINVAL, "bad mode");
+    if (mode != GRAV_MATRIX_FREE && c->stored_elem != (mode == GRAV_STORED_F64 ? 8 : 4))
+        return fail(GRAV_ESTATE, "stored G of the requested precision not present (grav_store_g)");
+    DeviceGuard dg(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const Geom& g = c->g;
+    double* dm = wsp<double>(c, c->lay.inv_dm);
+    double* r = wsp<double>(c, c->lay.inv_r);
+    double* dd = wsp<double>(c, c->lay.inv_dd);
+    double* rtry = wsp<double>(c, c->lay.inv_try);
+    double* scal = wsp<double>(c, c->lay.inv_scal);
+    double* part = wsp<double>(c, c->lay.dot_partial);
+    double* alpha = wsp<double>(c, c->lay.cg_x);
+    auto apply_G = [&](const double* u, double* d) {
+        return mode == GRAV_MATRIX_FREE ? grav_forward(c, u, d, stream) : grav_forward_stored(c, u, d, stream);
+    };
+    // ||out||^2 with out = a - t b (b may be NULL), summed over ranks when sharded; synchronises
+    auto norm2 = [&](const double* a_, double t, const double* b_, double* out, double* val) -> grav_status {
+        CK(launch_inv_residual(c, a_, t, b_, out, part, s), "inv_residual");
+        grav_status e = exchange(c, part, kDotBlocks, s);
+        if (e) return e;
+        CK(launch_inv_finish(c, part, scal, s), "inv_finish");
+        CK(cudaMemcpyAsync(val, scal, sizeof(double), cudaMemcpyDeviceToHost, s), "D2H norm");
+        CK(cudaStreamSynchronize(s), "sync");
+        return GRAV_OK;
+    };
+    double nd2 = 0.0, nr2 = 0.0;
+    if ((st = norm2(dobs, 0.0, nullptr, nullptr, &nd2))) return st;
+    if (mref) {
+        CK(cudaMemcpyAsync(m, mref, g.M * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy m_ref");
+        if ((st = apply_G(m, dd))) return st;
+        if ((st = norm2(dobs, 1.0, dd, r, &nr2))) return st;
+    } else {
+        CK(cudaMemsetAsync(m, 0, g.M * sizeof(double), s), "zero m");
+        if ((st = norm2(dobs, 0.0, nullptr, r, &nr2))) return st;
+    }
+    const double dn = nd2 > 0.0 ? std::sqrt(nd2) : 1.0;
+    if (hist_host) hist_host[0] = std::sqrt(nr2) / dn;
+    int k = 0;
+    for (; k < max_outer; ++k) {
+        if (std::sqrt(nr2) / dn <= tol_outer) break;
+        st = grav_dataspace_cg(c, r, w, lambda, max_inner, tol_inner, mode, nullptr, alpha, dm, nullptr, nullptr, stream);
+        if (st) return st;
+        if ((st = apply_G(dm, dd))) return st;
+        double step = 1.0, n2 = 0.0;
+        bool ok = false;
+        for (int h = 0; h <= 10; ++h, step *= 0.5) {
+            if ((st = norm2(r, step, dd, rtry, &n2))) return st;
+            if (n2 < nr2) { ok = true; break; }
+        }
+        if (step_host) step_host[k] = ok ? step : 0.0;
+        if (!ok) break;                                   // no decrease along delta_m: stop with m_k
+        CK(launch_inv_axpy(c, step, dm, m, m, s), "inv_axpy");
+        CK(cudaMemcpyAsync(r, rtry, g.N * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy r");
+        nr2 = n2;
+        if (hist_host) hist_host[k + 1] = std::sqrt(nr2) / dn;
+    }
+    if (n_outer_host) *n_outer_host = k;
+    if (dpred) {    // d_pred = d_obs - r
+        CK(launch_inv_residual(c, dobs, 1.0, r, dpred, part, s), "inv_residual");
+    }
     return GRAV_OK;
 }
 

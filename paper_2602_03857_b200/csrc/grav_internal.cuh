@@ -47,7 +47,7 @@ struct CgScalars {
 
 struct WsLayout {
     size_t cnode, tnode, fwd_partial, adj_partial, gcell, cg_x, cg_r, cg_p, cg_q, cg_w, dot_partial, scalars,
-        stage_m, stage_n, stage_hist, matfree_end, gemvt_partial, gstore;
+        stage_m, stage_n, stage_hist, inv_dm, inv_r, inv_dd, inv_try, inv_scal, matfree_end, gemvt_partial, gstore;
 };
 
 }  // namespace grav
@@ -107,6 +107,11 @@ cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double 
 cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
 cudaError_t launch_scale_cells(grav_ctx* c, double* g, const double* w, cudaStream_t s);
 int gemvt_chunks(long long N);
+// --- invert.cu : vector kernels of the outer model-update loop
+cudaError_t launch_inv_residual(grav_ctx* c, const double* r, double s, const double* dd, double* out, double* partial,
+                                cudaStream_t st);
+cudaError_t launch_inv_finish(grav_ctx* c, const double* partial, double* scalar, cudaStream_t st);
+cudaError_t launch_inv_axpy(grav_ctx* c, double a, const double* x, const double* y0, double* y, cudaStream_t st);
 cudaError_t init_forward_kernels();
 cudaError_t init_adjoint_kernels();
 cudaError_t init_stored_kernels();

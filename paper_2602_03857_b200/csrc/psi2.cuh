@@ -21,8 +21,11 @@
 
 namespace grav {
 
-constexpr int kLog2Bits = 8;
-constexpr int kLog2N = 1 << kLog2Bits;          // 256 mantissa intervals
+#ifndef GRAV_LOG2BITS
+#define GRAV_LOG2BITS 8
+#endif
+constexpr int kLog2Bits = GRAV_LOG2BITS;        // 8: |r| <= 2^-9, Taylor to r^5;  10: |r| <= 2^-11, Taylor to r^4
+constexpr int kLog2N = 1 << kLog2Bits;          // mantissa intervals
 constexpr int kAtan2K = 256;                    // c_j = j / 256, j = 0..256
 constexpr int kAtan2N = kAtan2K + 2;            // +1 slack entry for the seed's 2^-20 error at q = 1
 constexpr int kTab2Entries = kLog2N + kAtan2N;  // log entries first, then atan entries
@@ -83,14 +86,14 @@ struct Psi2TabView {
 // ln(a / 2^k0) for 0 < a < 2^1000 (finite garbage for a == 0: reading C6, the caller multiplies it by an exact 0).
 GRAV_HOSTDEV double log2_fast(const Psi2TabView& tb, double a) {
     const int hw = hi_word(a);
-    const unsigned mbits = (unsigned)hw & 0x000ff000u;                       // mantissa bits 19..12
+    const unsigned mbits = (unsigned)hw & (0x000fffffu & ~((1u << (20 - kLog2Bits)) - 1u));   // top mantissa bits
 #ifdef __CUDA_ARCH__
     // byte offset = idx * (16 << shift) = mbits >> (12 - 4 - shift): one shift-and-add on top of the base address
     // written as a high multiply by a power of two so that ptxas folds shift and base add into one LEA.HI
     const double2 ent = *reinterpret_cast<const double2*>(reinterpret_cast<const char*>(tb.base) +
-                                                          __umulhi(mbits, 1u << (32 - (8 - kRepShift))));
+                                                          __umulhi(mbits, 1u << (32 - (20 - kLog2Bits - 4 - kRepShift))));
 #else
-    const double2 ent = tb.base[(mbits >> 12) << tb.shift];
+    const double2 ent = tb.base[(mbits >> (20 - kLog2Bits)) << tb.shift];
 #endif
     const int e = (hw >> 20) - tb.k.ebias;                                   // a > 0: sign bit clear
     const double invc = make_double(hi_word(ent.x) - (e << 20), lo_word(ent.x));   // invc 2^-(e + k0): one IMAD
@@ -101,8 +104,13 @@ GRAV_HOSTDEV double log2_fast(const Psi2TabView& tb, double a) {
 #endif
     const double r = fma(a, invc, -1.0);
     const double r2 = r * r;
-    double q = fma(r, tb.k.l5, -0.25);
-    q = fma(q, r, tb.k.l3);
+    double q;
+    if (kLog2Bits >= 10) {
+        q = fma(r, -0.25, tb.k.l3);          // truncation r^5/5 <= 2^-55/5 = 5.5e-18
+    } else {
+        q = fma(r, tb.k.l5, -0.25);          // truncation r^6/6 <= 2^-54/6 = 9.3e-18
+        q = fma(q, r, tb.k.l3);
+    }
     q = fma(q, r, -0.5);
     const double p = fma(r2, q, r);
     const double base = fma(ed, tb.k.ln2, ent.y);

@@ -11,6 +11,7 @@
 // form_A / cholesky: explicit N x N data-space system for tiny N (BASELINE.json config 1).
 #include "grav_internal.cuh"
 #include "psi.cuh"
+#include "psi2.cuh"
 
 namespace grav {
 
@@ -18,7 +19,7 @@ namespace grav {
 // Flattened "layer" index q = cc*nzp + c over cell columns cc = i*ny + j and node layers c = 0..nz.
 // A warp owns 32 consecutive q starting at 31*warp; lane l < 31 outputs the prism (cc, k=c) if c < nz.
 template <bool FAST>
-__device__ __forceinline__ double layer_value(const Geom& g, const PsiTabView& tb, long long q, long long nq, double xo,
+__device__ __forceinline__ double layer_value(const Geom& g, const Psi2TabView& tb, long long q, long long nq, double xo,
                                               double yo, double zo, int& cc, int& c) {
     q = q < nq ? q : nq - 1;
     cc = (int)(q / g.nzp);
@@ -32,10 +33,10 @@ __device__ __forceinline__ double layer_value(const Geom& g, const PsiTabView& t
     if (FAST) {
         const PsiColumn c11 = psi_column(X1, Y1), c21 = psi_column(X2, Y1), c12 = psi_column(X1, Y2),
                         c22 = psi_column(X2, Y2);
-        v = c11.s * psi_fast(tb, c11, Z);
-        v = fma(-c21.s, psi_fast(tb, c21, Z), v);
-        v = fma(-c12.s, psi_fast(tb, c12, Z), v);
-        v = fma(c22.s, psi_fast(tb, c22, Z), v);
+        v = c11.s * psi2_fast(tb, c11, Z);
+        v = fma(-c21.s, psi2_fast(tb, c21, Z), v);
+        v = fma(-c12.s, psi2_fast(tb, c12, Z), v);
+        v = fma(c22.s, psi2_fast(tb, c22, Z), v);
     } else {
         v = psi_libm(X1, Y1, Z, X1 * Y1, fma(Y1, Y1, X1 * X1));
         v -= psi_libm(X2, Y1, Z, X2 * Y1, fma(Y1, Y1, X2 * X2));
@@ -46,10 +47,10 @@ __device__ __forceinline__ double layer_value(const Geom& g, const PsiTabView& t
 }
 
 template <typename T, int TPB, bool FAST>
-__global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, PsiDev pd, T* __restrict__ G) {
+__global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, Psi2Dev pd, T* __restrict__ G) {
     extern __shared__ double2 s_tab[];
-    PsiTabView tb;
-    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
+    Psi2TabView tb;
+    if (FAST) tb = psi2_tables_to_smem(s_tab, pd);
     const long long nq = (long long)g.nx * g.ny * g.nzp;
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * TPB + threadIdx.x) >> 5;
@@ -67,12 +68,12 @@ __global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, PsiDev pd, T* __r
 }
 
 template <int TPB, bool FAST>
-__global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, PsiDev pd, const double* __restrict__ w,
+__global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, Psi2Dev pd, const double* __restrict__ w,
                                                          double* __restrict__ diag) {
     extern __shared__ double2 s_tab[];
     __shared__ double sh[TPB];
-    PsiTabView tb;
-    if (FAST) tb = psi_tables_to_smem(s_tab, pd);
+    Psi2TabView tb;
+    if (FAST) tb = psi2_tables_to_smem(s_tab, pd);
     const long long nq = (long long)g.nx * g.ny * g.nzp;
     const int lane = threadIdx.x & 31;
     const int warp_in_block = threadIdx.x >> 5;
@@ -275,20 +276,20 @@ static unsigned pair_blocks(const Geom& g, int tpb) {
 }
 
 cudaError_t init_stored_kernels() {
-    cudaError_t e = cudaFuncSetAttribute(tabulate_kernel<double, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tabulate_kernel<float, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(gram_diag_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTabSmemBytes);
+    cudaError_t e = cudaFuncSetAttribute(tabulate_kernel<double, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tabulate_kernel<float, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gram_diag_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
     return e;
 }
 
 cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
     dim3 grid(pair_blocks(c->g, 256), (unsigned)(c->g.N < 65535 ? c->g.N : 65535));
     if (c->psi_variant == 0) {
-        if (elem == 8) tabulate_kernel<double, 256, true><<<grid, 256, kTabSmemBytes, s>>>(c->g, c->pd, (double*)G);
-        else tabulate_kernel<float, 256, true><<<grid, 256, kTabSmemBytes, s>>>(c->g, c->pd, (float*)G);
+        if (elem == 8) tabulate_kernel<double, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (double*)G);
+        else tabulate_kernel<float, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (float*)G);
     } else {
-        if (elem == 8) tabulate_kernel<double, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd, (double*)G);
-        else tabulate_kernel<float, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd, (float*)G);
+        if (elem == 8) tabulate_kernel<double, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd2, (double*)G);
+        else tabulate_kernel<float, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd2, (float*)G);
     }
     c->launches++;
     return cudaGetLastError();
@@ -296,8 +297,8 @@ cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
 
 cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
     unsigned blocks = (unsigned)(c->g.N < (1 << 20) ? c->g.N : (1 << 20));
-    if (c->psi_variant == 0) gram_diag_kernel<256, true><<<blocks, 256, kTabSmemBytes, s>>>(c->g, c->pd, w, diag);
-    else gram_diag_kernel<256, false><<<blocks, 256, 0, s>>>(c->g, c->pd, w, diag);
+    if (c->psi_variant == 0) gram_diag_kernel<256, true><<<blocks, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, w, diag);
+    else gram_diag_kernel<256, false><<<blocks, 256, 0, s>>>(c->g, c->pd2, w, diag);
     c->launches++;
     return cudaGetLastError();
 }

@@ -107,7 +107,7 @@ def _box(m3, i0, i1, j0, j1, k0, k1, val, add=False):
 
 
 def make(cfg: int) -> Workload:
-    """BASELINE.json configs 1..5 (1-based), with SURVEY.md App. B's concrete choices."""
+    """BASELINE.json configs 1..5 (1-based), with SURVEY.md App. B's concrete choices; 6 = the paper's Table 1 shape."""
     if cfg == 1:
         nx, ny, nz, h = 16, 16, 8, 50.0
         xn, yn, zn = _mesh(nx, ny, nz, h)
@@ -177,6 +177,22 @@ def make(cfg: int) -> Workload:
             dyke[90:140, max(j0, 0):max(min(j0 + 3, ny), 0), k] = True
         m3[dyke] += 300.0
         return Workload("cfg5_largest", 5, nx, ny, nz, h, xn, yn, zn, xo, yo, zo, m3.ravel(), 0.02, 50, z0=h / 2)
+    if cfg == 6:
+        # Not a BASELINE.json config: the SHAPE of the paper's largest single-GPU benchmark (Table 1, P:168-178;
+        # 2,601 stations x 3.28e6 cells, dense Float32 G = 34.13 GB), used by `bench.py --paper-shape` as the
+        # one point of contact with the paper's own wall-clock numbers.  The paper's model is
+        # not available; two +1000 kg/m^3 blocks stand in for its two-body synthetic.
+        nx, ny, nz, h = 160, 160, 128, 100.0
+        xn, yn, zn = _mesh(nx, ny, nz, h)
+        ns = 51
+        xs = (np.arange(ns) + 0.5) * (nx * h / ns)
+        X, Y = np.meshgrid(xs, xs, indexing="ij")
+        xo, yo, zo = X.ravel().copy(), Y.ravel().copy(), np.full(ns * ns, -1.0)
+        m3 = np.zeros((nx, ny, nz))
+        _box(m3, 40, 59, 60, 99, 10, 39, 1000.0)
+        _box(m3, 100, 119, 60, 99, 20, 59, 1000.0)
+        return Workload("paper_table1_shape", 6, nx, ny, nz, h, xn, yn, zn, xo, yo, zo, m3.ravel(), 0.01, 20,
+                        z0=h / 2)
     raise ValueError(f"unknown config {cfg}")
 
 

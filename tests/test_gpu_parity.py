@@ -271,6 +271,66 @@ def test_libm_variant_matches(cfg1):
     ctx.close()
 
 
+@pytest.mark.parametrize("shape", [(9, 7, 12, 700), (3, 4, 70, 300), (2, 2, 1100, 40)])
+def test_launch_variants_against_oracle(shape):
+    """Every forward / adjoint launch variant (staged and unstaged z-stream, first- and second-generation Psi
+    evaluator, every KC) against the oracle on a ragged case spanning several station tiles, several staged
+    column tiles and a column deeper than the stage buffer (nz + 1 > 1024: unstaged fallback)."""
+    nx, ny, nz, nobs = shape
+    wl = workloads.make_custom(nx, ny, nz, 17.0, nobs, seed=5 + nz, topo_amp=25.0)
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    rng = np.random.default_rng(nz)
+    u, v = rng.standard_normal(wl.M), rng.standard_normal(wl.N)
+    d_ref = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
+    g_ref = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)
+    ctx = make_ctx(wl)
+    for variant in range(6):
+        ctx.set_tuning(0, variant)
+        ctx.set_tuning(1, variant)
+        assert relmax(host(ctx.forward(dev(u))), d_ref) <= TOL_OP, f"forward variant {variant}"
+        assert relmax(host(ctx.adjoint(dev(v))), g_ref) <= TOL_OP, f"adjoint variant {variant}"
+    ctx.close()
+
+
+def test_outer_loop_cfg1(cfg1, c1):
+    """grav_invert (readings R1-R4) against oracle.invert on config 1, matrix-free and stored G,
+    with and without a reference model.  (a) inner CG capped at 8 iterations (no tolerance decision): three updates,
+    m, d_pred, residual history and steps at 1e-8.  (b) inner tolerance decides the iteration count: the tolerance is
+    placed midway (in log) between two consecutive oracle residuals, so both sides must stop after the same
+    iteration.  (c) the paper's settings (30 x 20, 1e-4) run to completion: compare the invariants."""
+    wl, G, w, lam, d = cfg1["wl"], cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
+    mref = np.full(wl.M, 2.5)
+    c1.store_g()
+    wd = dev(w)
+    for mode in (0, 1):
+        for mr in (None, mref):
+            m_o, dp_o, hist_o, steps_o = oracle.invert(G, w, lam, d, mref=mr, max_outer=3, max_inner=8, tol_outer=0.0,
+                                                       tol_inner=0.0)
+            out = c1.invert(dev(d), wd, lam, mref=None if mr is None else dev(mr), max_outer=3, max_inner=8,
+                            tol_outer=0.0, tol_inner=0.0, mode=mode)
+            assert out["n_outer"] == 3 and out["steps"].tolist() == steps_o.tolist()
+            assert relmax(host(out["m"]), m_o) <= TOL_CG
+            assert relmax(host(out["dpred"]), dp_o) <= TOL_CG
+            assert np.allclose(out["hist"], hist_o, rtol=1e-8)
+    # (b) tolerance-decided inner stop
+    _, hist, _ = oracle.cg(w, lam, d, 14, G=G)
+    rel = hist / hist[0]
+    assert rel[10] > 1.3 * rel[11]
+    tol = float(np.sqrt(rel[10] * rel[11]))
+    m_o, _, hist_o, _ = oracle.invert(G, w, lam, d, max_outer=1, max_inner=20, tol_outer=0.0, tol_inner=tol)
+    m_cap, _, _, _ = oracle.invert(G, w, lam, d, max_outer=1, max_inner=11, tol_outer=0.0, tol_inner=0.0)
+    assert np.array_equal(m_o, m_cap)                       # the oracle stopped after iteration 11
+    out = c1.invert(dev(d), wd, lam, max_outer=1, max_inner=20, tol_outer=0.0, tol_inner=tol)
+    assert relmax(host(out["m"]), m_o) <= TOL_CG and np.allclose(out["hist"], hist_o, rtol=1e-8)
+    # (c) the paper's settings
+    out = c1.invert(dev(d), wd, lam, mref=dev(mref))
+    m, dp = host(out["m"]), host(out["dpred"])
+    assert np.all(np.diff(out["hist"]) < 0) and np.all(out["steps"] > 0)
+    assert out["n_outer"] == 30 or out["hist"][-1] <= 1e-4
+    assert relmax(dp, oracle.dense_matvec(G, m)) <= 1e-9
+    assert np.linalg.norm(d - dp) / np.linalg.norm(d) == pytest.approx(out["hist"][-1], rel=1e-8)
+
+
 def test_allreduce_hook_placement(cfg1):
     """Observation sharding (include/grav.h: grav_set_allreduce).  Two IDENTICAL ranks, each holding the same
     stations S, form the global system [G_S; G_S]; its all-reduce is "multiply by 2".  By symmetry the sharded CG must
