@@ -225,7 +225,7 @@ def paper_shape_leg(local, matrix_free=False):
     t2 = time.perf_counter()
     res = {"workload": wl.name, "prisms": wl.M, "stations": wl.N, "g_bytes_f32": float(wl.N) * wl.M * 4,
            "build_s": t1 - t0, "inversion_s": t2 - t1, "total_s": t2 - t0, "outer_updates": out["n_outer"],
-           "rel_residual": float(out["hist"][-1]), "gpu_launches": ctx.launches - l0, "lambda": lam,
+           "stop": out["stop"], "rel_residual": float(out["hist"][-1]), "gpu_launches": ctx.launches - l0, "lambda": lam,
            "paper_context": {"total_s_1xA100_f32": 63.88, "total_s_cpu_epyc7h12": 1007.46,
                              "source": "PAPER.md Table 1 (P:168-178), 3.28e6 cells x 2,601 stations"}}
     if matrix_free:

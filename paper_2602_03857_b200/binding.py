@@ -249,7 +249,8 @@ class GravContext:
                                      C.c_void_p(hist.ctypes.data), C.c_void_p(steps.ctypes.data), C.byref(n_outer),
                                      _stream()))
         k = n_outer.value
-        return dict(m=m, dpred=dpred, hist=hist[:k + 1], steps=steps[:k], n_outer=k)
+        stop = "tolerance" if hist[k] <= tol_outer else ("max_outer" if k == max_outer else "no_decrease")
+        return dict(m=m, dpred=dpred, hist=hist[:k + 1], steps=steps[:k], n_outer=k, stop=stop)
 
     def store_g(self, fp32=False):
         want = STORED_F32 if fp32 else STORED_F64

@@ -146,6 +146,7 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
             case 0:   // shipped: the plan's choice of KC (grav_api.cu make_plan)
                 if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
                 else if (p.adj_kc == 6) e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s);
+                else if (p.adj_kc == 8) e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s);
                 else e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s);
                 break;
             case 1: e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s); break;

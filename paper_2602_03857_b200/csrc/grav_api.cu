@@ -50,16 +50,17 @@ void make_plan(const Geom& g, Plan& p) {
     p.fwd_cols_per_chunk = ceil_div(g.ncol, want);
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
-    // KC nodes per thread: per-(thread, station) set-up (~22 issue cycles) is shared by KC evaluations (~115 each)
-    // but the column is padded to a multiple of KC; pick the cheapest of the compiled variants for this nz.
+    // KC nodes per thread: the per-(thread, station) set-up is shared by KC evaluations but the column is padded to a
+    // multiple of KC.  Measured scheduler cycles per warp-evaluation fit (119.5 + 25.6 / KC) x padding within 1 % for
+    // KC = 4, 5, 6, 8 at configs 3 and 5 (profiles/r1_tail_and_variants.md); pick the cheapest compiled variant.
     p.adj_tpb = 256;
     p.adj_kc = 4;
     double best = 1e300;
-    for (int kc = 4; kc <= 6; ++kc) {
-        const double cost = (115.0 + 22.0 / kc) * (double)(ceil_div(g.nzp, kc) * kc);
+    for (int kc : {4, 5, 6, 8}) {
+        const double cost = (119.5 + 25.6 / kc) * (double)(ceil_div(g.nzp, kc) * kc);
         if (cost < best) { best = cost; p.adj_kc = kc; }
     }
-    if (p.adj_kc == 6) p.adj_tpb = 128;
+    if (p.adj_kc >= 6) p.adj_tpb = 128;
     p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
     want = ceil_div(148 * 128, p.adj_blocks);

@@ -296,7 +296,7 @@ def test_outer_loop_cfg1(cfg1, c1):
     """grav_invert (readings R1-R4) against oracle.invert on config 1, matrix-free and stored G,
     with and without a reference model.  (a) inner CG capped at 8 iterations (no tolerance decision): three updates,
     m, d_pred, residual history and steps at 1e-8.  (b) inner tolerance decides the iteration count: the tolerance is
-    placed midway (in log) between two consecutive oracle residuals, so both sides must stop after the same
+    placed midway (in log) between two consecutive early oracle residuals, so both sides must stop after the same
     iteration.  (c) the paper's settings (30 x 20, 1e-4) run to completion: compare the invariants."""
     wl, G, w, lam, d = cfg1["wl"], cfg1["G"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
     mref = np.full(wl.M, 2.5)
@@ -313,13 +313,15 @@ def test_outer_loop_cfg1(cfg1, c1):
             assert relmax(host(out["dpred"]), dp_o) <= TOL_CG
             assert np.allclose(out["hist"], hist_o, rtol=1e-8)
     # (b) tolerance-decided inner stop
-    _, hist, _ = oracle.cg(w, lam, d, 14, G=G)
+    # (the decision has to fall early: this system has an isolated top eigenvalue and its CG iterates are chaotic from
+    #  k ~ 9 on - the oracle's own residual at k = 11 changes by 36 % when its sums are reversed)
+    _, hist, _ = oracle.cg(w, lam, d, 6, G=G)
     rel = hist / hist[0]
-    assert rel[10] > 1.3 * rel[11]
-    tol = float(np.sqrt(rel[10] * rel[11]))
+    assert rel[2] > 2.0 * rel[3] and rel[1] > rel[2]
+    tol = float(np.sqrt(rel[2] * rel[3]))
     m_o, _, hist_o, _ = oracle.invert(G, w, lam, d, max_outer=1, max_inner=20, tol_outer=0.0, tol_inner=tol)
-    m_cap, _, _, _ = oracle.invert(G, w, lam, d, max_outer=1, max_inner=11, tol_outer=0.0, tol_inner=0.0)
-    assert np.array_equal(m_o, m_cap)                       # the oracle stopped after iteration 11
+    m_cap, _, _, _ = oracle.invert(G, w, lam, d, max_outer=1, max_inner=3, tol_outer=0.0, tol_inner=0.0)
+    assert np.array_equal(m_o, m_cap)                       # the oracle stopped after iteration 3
     out = c1.invert(dev(d), wd, lam, max_outer=1, max_inner=20, tol_outer=0.0, tol_inner=tol)
     assert relmax(host(out["m"]), m_o) <= TOL_CG and np.allclose(out["hist"], hist_o, rtol=1e-8)
     # (c) the paper's settings
