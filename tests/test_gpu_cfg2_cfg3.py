@@ -146,3 +146,23 @@ def test_cfg3_stored_f32():
     print(f"cfg3 stored FP32 error: forward {e_f:.2e}, adjoint {e_a:.2e} (of max)")
     assert e_f <= 2e-7 and e_a <= 2e-7
     ctx.close()
+
+
+def test_cfg2_outer_loop_against_oracle(cfg2):
+    """grav_invert (readings R1-R4) at config 2 against oracle.invert with the oracle's dense G, with a
+    reference model, matrix-free and stored FP64 G: one update of 5 CG iterations and two updates of 3.  These stay
+    inside the prefix where the iterates are unique (protocol P2): the oracle's own result moves by <= 3e-12 when its G
+    is perturbed by 1e-13, whereas two updates of 5 iterations already move by 7e-8 (cond(A) = 2.2e4)."""
+    wl, G, w, lam, d, ctx = cfg2["wl"], cfg2["G"], cfg2["w"], cfg2["lam"], cfg2["d_obs"], cfg2["ctx"]
+    mref = np.full(wl.M, 1.5)
+    ctx.store_g()
+    for n_outer, n_inner in ((1, 5), (2, 3)):
+        m_o, dp_o, hist_o, steps_o = oracle.invert(G, w, lam, d, mref=mref, max_outer=n_outer, max_inner=n_inner,
+                                                   tol_outer=0.0, tol_inner=0.0)
+        for mode in (0, 1):
+            out = ctx.invert(dev(d), dev(w), lam, mref=dev(mref), max_outer=n_outer, max_inner=n_inner, tol_outer=0.0,
+                             tol_inner=0.0, mode=mode)
+            assert out["n_outer"] == n_outer and out["steps"].tolist() == steps_o.tolist()
+            assert relmax(host(out["m"]), m_o) <= TOL_CG
+            assert relmax(host(out["dpred"]), dp_o) <= TOL_CG
+            assert np.allclose(out["hist"], hist_o, rtol=1e-8)
