@@ -118,13 +118,11 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
 
 template <int TPB, int KC, int MINB, int EV = 1>
 static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
-    static bool inited = false;
     constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
-    if (!inited) {
-        cudaError_t e = cudaFuncSetAttribute(adjoint_nodes_kernel<TPB, KC, MINB, EV>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static unsigned long long smem_set = 0;
+    {
+        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, smem, c->device, &smem_set);
         if (e != cudaSuccess) return e;
-        inited = true;
     }
     const Plan& p = c->plan;
     const int ncg = (c->g.nzp + KC - 1) / KC;

@@ -177,13 +177,11 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
 // Launch variants (grav_debug_set_tuning(ctx, 0, v)); the default is the one measured fastest (profiles/).
 template <int TPB, int UNROLL, int MINB, int EV = 1>
 static cudaError_t fwd_launch_fast(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
-    static bool inited = false;
     constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
-    if (!inited) {
-        cudaError_t e = cudaFuncSetAttribute(forward_nodes_kernel<TPB, UNROLL, MINB, EV>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static unsigned long long smem_set = 0;
+    {
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_kernel<TPB, UNROLL, MINB, EV>, smem, c->device, &smem_set);
         if (e != cudaSuccess) return e;
-        inited = true;
     }
     const Plan& p = c->plan;
     dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);
@@ -195,13 +193,11 @@ static cudaError_t fwd_launch_fast(grav_ctx* c, const double2* cnode, double* pa
 template <int TPB, int UNROLL, int MINB, int EV = 2>
 static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
     if (c->g.nzp > kFwdStage) return fwd_launch_fast<TPB, UNROLL, MINB, EV>(c, cnode, partial, done, s);
-    static bool inited = false;
     constexpr size_t smem = (EV == 2 ? kTab2SmemBytes : kTabSmemBytes) + 2 * kFwdStage * sizeof(double2);
-    if (!inited) {
-        cudaError_t e = cudaFuncSetAttribute(forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static unsigned long long smem_set = 0;
+    {
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV>, smem, c->device, &smem_set);
         if (e != cudaSuccess) return e;
-        inited = true;
     }
     const Plan& p = c->plan;
     dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);

@@ -216,7 +216,7 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         if (c->pd.k0 > 900) c->pd.k0 = 900;
         if (c->pd.k0 < -900) c->pd.k0 = -900;
         c->pd.k = psi_consts_make(c->pd.k0);
-        static Psi2TablesHost tabs2;      // ~8 KB; regenerated per context (depends on k0)
+        Psi2TablesHost tabs2;             // ~8 KB; generated per context (depends on k0)
         psi2_tables_generate(&tabs2, c->pd.k0);
         c->pd2.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs2), ntab2));
         c->pd2.k = psi2_consts_make(c->pd.k0);

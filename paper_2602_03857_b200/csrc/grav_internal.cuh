@@ -72,6 +72,17 @@ struct grav_ctx {
 
 namespace grav {
 
+// Opt a kernel into > 48 KB of dynamic shared memory once per (kernel, device); thread-safe (the attribute is per
+// device, and setting it twice is harmless).
+template <class Kernel>
+inline cudaError_t ensure_dynamic_smem(Kernel kernel, size_t bytes, int device, unsigned long long* done_mask) {
+    const unsigned long long bit = 1ull << (device & 63);
+    if (__atomic_load_n(done_mask, __ATOMIC_ACQUIRE) & bit) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) __atomic_fetch_or(done_mask, bit, __ATOMIC_RELEASE);
+    return e;
+}
+
 // every launcher returns cudaGetLastError() of its launches and bumps ctx->launches
 // --- nodeops.cu
 cudaError_t launch_cell_to_node(grav_ctx* c, const double* u, const double* w_or_null, double* cnode, cudaStream_t s);
