@@ -30,7 +30,8 @@ UNIT = "pair evals/s"
 
 # FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
 # capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
-FP64_INST_PER_EVAL = {"forward_nodes": 46.0, "adjoint_nodes": 46.0}
+# 44 with the exponent-and-mantissa log table (used when the geometry admits it: all five configs), 46 otherwise
+FP64_INST_PER_EVAL = {True: 44.0, False: 46.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 5 from the committed `ncu --set full` capture
 # (profiles/r1_ncu_full_cfg5.md); None for other configs
 NCU_DRAM_BYTES = {5: {"forward_nodes": 76.6e6, "adjoint_nodes": 453.1e6}}
@@ -375,7 +376,8 @@ def run_ours(args):
 
     evals = float(Nloc) * Nn                     # node evaluations one launch of this rank processes
     dom, t_dom = ("forward_nodes", t_fwd) if t_fwd >= t_adj else ("adjoint_nodes", t_adj)
-    inst = FP64_INST_PER_EVAL[dom] * evals
+    per_eval = FP64_INST_PER_EVAL[ctx.log2d_binades > 0]
+    inst = per_eval * evals
     achieved = inst / (t_dom * 1e-3) / 1e12
     peak_nominal = 148 * FP64_LANES_PER_SM * 1.965e9 / 1e12
     probe_rate, _ = binding.fp64_peak_probe(local, 100000)
@@ -387,7 +389,7 @@ def run_ours(args):
                        f"DFMA-only probe in this run: {probe_rate / 1e12:.2f} T inst/s",
         "frac_of_probe": achieved / (probe_rate / 1e12),
         "frac_at_held_clock": achieved / (148 * FP64_LANES_PER_SM * clk * 1e6 / 1e12),
-        "fp64_inst_per_eval": FP64_INST_PER_EVAL[dom], "evals_per_launch": evals,
+        "fp64_inst_per_eval": per_eval, "log2d_binades": ctx.log2d_binades, "evals_per_launch": evals,
         "ms_forward": t_fwd, "ms_adjoint": t_adj,
         "pairs_per_s_forward": float(Nloc) * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": float(Nloc) * M / (t_adj * 1e-3),
     }

@@ -187,10 +187,17 @@ grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
  * csrc/psi.cuh). */
 double grav_debug_psi_fast_host(double X, double Y, double Z, int k0);
 /* The same for the second-generation evaluator of csrc/psi2.cuh (swap-free atan2 reduction, exponent folded into
- * the log table entry): returns Psi(X,Y,Z) + (X+Y)*k0*ln2. */
+ * the log table entry): returns Psi(X,Y,Z) + (X+Y)*k0*ln2.  Caches its tables per k0: not thread-safe. */
 double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0);
+/* The same with the logarithms taken from the exponent-and-mantissa ("2-D") table the kernels use when the geometry
+ * bounds their arguments (csrc/psi2.cuh, LOG2D); valid for arguments in [2^-80, 2^80).  Not thread-safe. */
+double grav_debug_psi2_log2d_host(double X, double Y, double Z, int k0);
 /* The global exponent offset k0 chosen for this context (2^k0 ~ survey scale). */
 int grav_debug_k0(const grav_ctx* ctx);
+/* Number of binades of the exponent-and-mantissa log table this context's kernels use, or 0 when the geometry does
+ * not bound the arguments of the logarithms (a station level with or inside the mesh, or a ratio above 2^40) and the
+ * kernels use the 256-entry table with explicit exponent handling instead. */
+int grav_debug_log2d_binades(const grav_ctx* ctx);
 
 /* Thread-local message of the last failure on this thread ("" if none). */
 const char* grav_last_error(void);

@@ -21,8 +21,8 @@ EXPORTS = [
     "grav_forward", "grav_adjoint", "grav_depth_weights", "grav_dataspace_cg", "grav_store_g",
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
-    "grav_fp64_peak_probe", "grav_fp64_mix_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host",
-    "grav_debug_k0", "grav_debug_set_tuning", "grav_set_allreduce",
+    "grav_fp64_peak_probe", "grav_fp64_mix_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host", "grav_debug_psi2_log2d_host",
+    "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_set_tuning", "grav_set_allreduce",
 ]
 
 # int fn(double* buf_dev, long long count, void* stream, void* user)   (include/grav.h: grav_allreduce_fn)
@@ -96,12 +96,16 @@ def load():
     L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
     L.grav_debug_psi2_fast_host.restype = d
     L.grav_debug_psi2_fast_host.argtypes = [d, d, d, i]
+    L.grav_debug_psi2_log2d_host.restype = d
+    L.grav_debug_psi2_log2d_host.argtypes = [d, d, d, i]
     L.grav_debug_set_tuning.restype = i
     L.grav_debug_set_tuning.argtypes = [vp, i, i]
     L.grav_set_allreduce.restype = i
     L.grav_set_allreduce.argtypes = [vp, ALLREDUCE_FN, vp]
     L.grav_debug_k0.restype = i
     L.grav_debug_k0.argtypes = [vp]
+    L.grav_debug_log2d_binades.restype = i
+    L.grav_debug_log2d_binades.argtypes = [vp]
     L.grav_last_error.restype = C.c_char_p
     L.grav_last_error.argtypes = []
     _lib = L
@@ -343,13 +347,19 @@ class GravContext:
         return int(self._lib.grav_debug_k0(self._h))
 
     @property
+    def log2d_binades(self):
+        return int(self._lib.grav_debug_log2d_binades(self._h))
+
+    @property
     def launches(self):
         return int(self._lib.grav_launch_count(self._h))
 
 
 def psi_fast_host(X, Y, Z, k0=0, gen=1):
-    """Host emulation of the device Psi evaluators (diagnostic; needs no GPU): gen 1 = psi.cuh, 2 = psi2.cuh."""
-    fn = load().grav_debug_psi2_fast_host if gen == 2 else load().grav_debug_psi_fast_host
+    """Host emulation of the device Psi evaluators (diagnostic; needs no GPU): gen 1 = psi.cuh, 2 = psi2.cuh,
+    3 = psi2.cuh with the 2-D log table."""
+    fn = {1: load().grav_debug_psi_fast_host, 2: load().grav_debug_psi2_fast_host,
+          3: load().grav_debug_psi2_log2d_host}[gen]
     return float(fn(float(X), float(Y), float(Z), int(k0)))
 
 

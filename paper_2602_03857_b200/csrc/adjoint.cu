@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     Psi2TabView tb2;
     if (EV == 1) tb = psi_tables_to_smem(s_tab, pd);
     if (EV == 2) tb2 = psi2_tables_to_smem(s_tab, pd2);
+    if (EV == 3) tb2 = psi2_tables_to_smem_2d(s_tab, pd2);
     const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long nthreads = (long long)g.ncol * ncg;
     const bool valid = t < nthreads;
@@ -77,7 +78,9 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
                 const double vs = o.w * pc.s;
 #pragma unroll
                 for (int k = 0; k < KC; ++k)
-                    acc[k] = fma(vs, EV == 1 ? psi_fast(tb, pc, zc[k] - o.z) : psi2_fast(tb2, pc, zc[k] - o.z), acc[k]);
+                    acc[k] = fma(vs, EV == 1 ? psi_fast(tb, pc, zc[k] - o.z)
+                                             : (EV == 3 ? psi2_fast_t<true>(tb2, pc, zc[k] - o.z)
+                                                        : psi2_fast(tb2, pc, zc[k] - o.z)), acc[k]);
             } else {
                 const double XY = X * Y;
                 const double Q = fma(Y, Y, X * X);
@@ -118,10 +121,14 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
 
 template <int TPB, int KC, int MINB, int EV = 1>
 static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
-    constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
+    if (EV == 3 && !c->pd2.tab2d) return cudaErrorInvalidValue;      // geometry outside the 2-D log table
+    // EV == 3: the opt-in is sized for the largest 2-D table, the launch for this context's table
+    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096
+                                        : (EV == 2 ? kTab2SmemBytes : kTabSmemBytes);
+    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
     static unsigned long long smem_set = 0;
     {
-        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, smem, c->device, &smem_set);
+        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, smem_max, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
     const Plan& p = c->plan;
@@ -142,16 +149,26 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
         switch (c->tune[1]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
             default:
             case 0:   // shipped: the plan's choice of KC (grav_api.cu make_plan)
-                if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
+                if (p.log2d) {
+                    if (p.adj_kc == 4) e = adj_launch_fast<512, 4, 1, 3>(c, v, partial, done, s);
+                    else if (p.adj_kc == 5) e = adj_launch_fast<512, 5, 1, 3>(c, v, partial, done, s);
+                    else if (p.adj_kc == 6) e = adj_launch_fast<256, 6, 1, 3>(c, v, partial, done, s);
+                    else e = adj_launch_fast<256, 8, 1, 3>(c, v, partial, done, s);
+                } else if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
                 else if (p.adj_kc == 6) e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s);
                 else if (p.adj_kc == 8) e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s);
                 else e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s);
                 break;
             case 1: e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s); break;
+            case 10: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
             case 2: e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s); break;
             case 3: e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s); break;
             case 4: e = adj_launch_fast<128, 4, 4, 1>(c, v, partial, done, s); break;          // first generation
             case 5: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
+            case 6: e = adj_launch_fast<512, 4, 1, 3>(c, v, partial, done, s); break;          // 2-D log table
+            case 7: e = adj_launch_fast<256, 8, 1, 3>(c, v, partial, done, s); break;
+            case 8: e = adj_launch_fast<512, 5, 1, 3>(c, v, partial, done, s); break;
+            case 9: e = adj_launch_fast<256, 6, 1, 3>(c, v, partial, done, s); break;
         }
     } else {
         const int ncg4 = (c->g.nzp + 3) / 4;

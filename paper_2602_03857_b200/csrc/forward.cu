@@ -95,6 +95,7 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g,
     Psi2TabView tb2;
     double2* s_stage;
     if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); s_stage = s_tab + kTabEntries * kRep; }
+    else if (EV == 3) { tb2 = psi2_tables_to_smem_2d(s_tab, pd2); s_stage = s_tab + psi2_log2d_smem_entries(pd2); }
     else { tb2 = psi2_tables_to_smem(s_tab, pd2); s_stage = s_tab + kTab2Entries * kRep; }
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
@@ -129,7 +130,8 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g,
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = sc[c];
                 const double Z = cz.y - zo;
-                colacc = fma(cz.x, EV == 1 ? psi_fast(tb, pc, Z) : psi2_fast(tb2, pc, Z), colacc);
+                colacc = fma(cz.x, EV == 1 ? psi_fast(tb, pc, Z)
+                                           : (EV == 3 ? psi2_fast_t<true>(tb2, pc, Z) : psi2_fast(tb2, pc, Z)), colacc);
             }
             acc = fma(colacc, pc.s, acc);
             if (++b == g.nyp) {
@@ -192,11 +194,16 @@ static cudaError_t fwd_launch_fast(grav_ctx* c, const double2* cnode, double* pa
 
 template <int TPB, int UNROLL, int MINB, int EV = 2>
 static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
-    if (c->g.nzp > kFwdStage) return fwd_launch_fast<TPB, UNROLL, MINB, EV>(c, cnode, partial, done, s);
-    constexpr size_t smem = (EV == 2 ? kTab2SmemBytes : kTabSmemBytes) + 2 * kFwdStage * sizeof(double2);
+    if (c->g.nzp > kFwdStage) return fwd_launch_fast<TPB, UNROLL, MINB, EV == 3 ? 2 : EV>(c, cnode, partial, done, s);
+    if (EV == 3 && !c->pd2.tab2d) return cudaErrorInvalidValue;      // geometry outside the 2-D log table
+    constexpr size_t stage = 2 * kFwdStage * sizeof(double2);
+    // EV == 3: the opt-in is sized for the largest 2-D table, the launch for this context's table
+    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 + stage
+                                        : (EV == 2 ? kTab2SmemBytes : kTabSmemBytes) + stage;
+    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 + stage : smem_max;
     static unsigned long long smem_set = 0;
     {
-        cudaError_t e = ensure_dynamic_smem(forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV>, smem, c->device, &smem_set);
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV>, smem_max, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
     const Plan& p = c->plan;
@@ -215,12 +222,18 @@ cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* part
     if (c->psi_variant == 0) {
         switch (c->tune[0]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
             default:
-            case 0: e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s); break;      // shipped
+            case 0:   // shipped: 2-D log table when the geometry admits it (grav_api.cu), else the 256-entry table
+                if (p.log2d) e = fwd_launch_staged<512, 8, 1, 3>(c, cnode, partial, done, s);
+                else e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s);
+                break;
+            case 8: e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s); break;
             case 1: e = fwd_launch_staged<256, 4, 2>(c, cnode, partial, done, s); break;
             case 2: e = fwd_launch_fast<256, 4, 2, 2>(c, cnode, partial, done, s); break;     // psi2, unstaged
             case 3: e = fwd_launch_fast<256, 8, 2, 2>(c, cnode, partial, done, s); break;
             case 4: e = fwd_launch_fast<128, 2, 4, 1>(c, cnode, partial, done, s); break;     // first generation
             case 5: e = fwd_launch_staged<512, 8, 1>(c, cnode, partial, done, s); break;
+            case 6: e = fwd_launch_staged<512, 8, 1, 3>(c, cnode, partial, done, s); break;     // 2-D log table
+            case 7: e = fwd_launch_staged<512, 4, 1, 3>(c, cnode, partial, done, s); break;
         }
     } else {
         dim3 grid((unsigned)((c->g.N + 127) / 128), p.fwd_nchunk);

@@ -1,9 +1,11 @@
 // grav_api.cu -- the C ABI of include/grav.h: context, workspace layout, call sequencing.  No arithmetic of the
 // method lives here except the order in which kernels are enqueued.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <new>
 #include <vector>
 
@@ -33,13 +35,15 @@ size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Launch plan: enough blocks to fill 148 SMs several times over, fixed per context => deterministic sums.
-void make_plan(const Geom& g, Plan& p) {
+// log2d: the context's geometry admits the 2-D log table (psi2.cuh LOG2D): kernels of 512 / 256 threads, 1 block per SM.
+void make_plan(const Geom& g, bool log2d, Plan& p) {
+    p.log2d = log2d ? 1 : 0;
     // Blocks of one launch all take the same time, so a grid of W.f waves of resident blocks costs ceil(W.f) waves:
     // with ~5 waves (the first plan) up to 18 % of the launch was tail.  ~100 blocks per SM keeps the tail <= 2-3 %
     // (profiles/r1_tail_and_variants.md); the price is a larger partial buffer (<= 40 MB), read once.
-    const int target_blocks = 148 * 96;
-    // forward: 256 stations per block; split the node columns into chunks when the station tiles are few
-    p.fwd_tpb = 256;
+    const int target_blocks = log2d ? 148 * 48 : 148 * 96;      // ~48 waves either way
+    // forward: 256 (512) stations per block; split the node columns into chunks when the station tiles are few
+    p.fwd_tpb = log2d ? 512 : 256;
     p.fwd_obs_per_thread = 1;
     p.fwd_tiles = ceil_div(g.N, p.fwd_tpb * p.fwd_obs_per_thread);
     int want = ceil_div(target_blocks, p.fwd_tiles);
@@ -53,17 +57,20 @@ void make_plan(const Geom& g, Plan& p) {
     // KC nodes per thread: the per-(thread, station) set-up is shared by KC evaluations but the column is padded to a
     // multiple of KC.  Measured scheduler cycles per warp-evaluation fit (119.5 + 25.6 / KC) x padding within 1 % for
     // KC = 4, 5, 6, 8 at configs 3 and 5 (profiles/r1_tail_and_variants.md); pick the cheapest compiled variant.
+    // With the 2-D log table the fit is (108.5 + 32.8 / KC) x padding.
     p.adj_tpb = 256;
     p.adj_kc = 4;
     double best = 1e300;
     for (int kc : {4, 5, 6, 8}) {
-        const double cost = (119.5 + 25.6 / kc) * (double)(ceil_div(g.nzp, kc) * kc);
+        const double per_eval = log2d ? 108.5 + 32.8 / kc : 119.5 + 25.6 / kc;
+        const double cost = per_eval * (double)(ceil_div(g.nzp, kc) * kc);
         if (cost < best) { best = cost; p.adj_kc = kc; }
     }
-    if (p.adj_kc >= 6) p.adj_tpb = 128;
+    if (log2d) p.adj_tpb = p.adj_kc <= 5 ? 512 : 256;
+    else if (p.adj_kc >= 6) p.adj_tpb = 128;
     p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
-    want = ceil_div(148 * 128, p.adj_blocks);
+    want = ceil_div(log2d ? 148 * 48 : 148 * 128, p.adj_blocks);
     while (want > 1 && (double)want * 2.0 * g.Nn * 8.0 > 256e6) --want;   // [hi|lo] partial planes <= 256 MB
     int maxchunk = ceil_div(g.N, 64);
     if (want > maxchunk) want = maxchunk;
@@ -187,7 +194,8 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
 
     const size_t ntab = sizeof(PsiTablesHost) / sizeof(double);
     const size_t ntab2 = sizeof(Psi2TablesHost) / sizeof(double);
-    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2 + 8 * 32;   // each array 256-byte aligned
+    const size_t ntab2d = (size_t)kLog2dMaxBinades * 256 * 2;
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2 + ntab2d + 9 * 32;   // each array 256-byte aligned
     std::vector<double> host;
     try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
     void* dev = nullptr;
@@ -220,6 +228,34 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         psi2_tables_generate(&tabs2, c->pd.k0);
         c->pd2.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs2), ntab2));
         c->pd2.k = psi2_consts_make(c->pd.k0);
+        // 2-D log table (experimental variant): arguments a = R + Y obey Zmin^2 / (2 Rmax) <= a <= 2 Rmax, with Zmin the
+        // smallest vertical station-node distance and Rmax the largest station-node distance
+        c->pd2.tab2d = nullptr; c->pd2.nb2d = 0; c->pd2.emin2d_biased = 0;
+        double zmin = INFINITY, r2max = 0.0;
+        for (long long i = 0; i < nobs; ++i) {
+            const double dx = std::max(std::fabs(xn[0] - ox[i]), std::fabs(xn[nx] - ox[i]));
+            const double dy = std::max(std::fabs(yn[0] - oy[i]), std::fabs(yn[ny] - oy[i]));
+            const double dz = std::max(std::fabs(zn[0] - oz[i]), std::fabs(zn[nz] - oz[i]));
+            r2max = std::max(r2max, dx * dx + dy * dy + dz * dz);
+            const double* lb = std::lower_bound(zn, zn + nz + 1, oz[i]);
+            if (lb != zn + nz + 1) zmin = std::min(zmin, std::fabs(*lb - oz[i]));
+            if (lb != zn) zmin = std::min(zmin, std::fabs(*(lb - 1) - oz[i]));
+        }
+        const double rmax = std::sqrt(r2max);
+        if (zmin > 0.0 && std::isfinite(zmin) && rmax > 0.0 && std::isfinite(rmax)) {
+            // one binade of slack below for the rounding of R in R + Y (needs zmin^2 / rmax >> rmax 2^-53, implied
+            // by the binade limit); the upper bound 2 Rmax is rigorous up to the rounding covered by the 1e-12
+            const int elo = (int)std::ilogb(zmin * zmin / (2.0 * rmax)) - 1;
+            const int ehi = (int)std::ilogb(2.0 * rmax * (1.0 + 1e-12));
+            const int nb = ehi - elo + 1;
+            if (nb <= kLog2dMaxBinades && elo > -900 && ehi < 900) {
+                std::vector<double2> t2d((size_t)nb * 256);
+                psi2_log2d_generate(t2d.data(), c->pd.k0, elo, nb);
+                c->pd2.tab2d = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(t2d.data()), (size_t)nb * 512));
+                c->pd2.nb2d = nb;
+                c->pd2.emin2d_biased = elo + 1023;
+            }
+        }
         c->psi_variant = 0;
     }
     e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
@@ -229,7 +265,7 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     if (e == cudaSuccess) e = init_adjoint_kernels();
     if (e == cudaSuccess) e = init_stored_kernels();
     if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaFuncSetAttribute"); }
-    make_plan(g, c->plan);
+    make_plan(g, c->pd2.tab2d != nullptr, c->plan);
     make_layout(g, c->plan, c->lay);
     *out = c;
     return GRAV_OK;
@@ -290,6 +326,8 @@ grav_status grav_debug_set_tuning(grav_ctx* c, int which, int value) {
 
 int grav_debug_k0(const grav_ctx* c) { return c ? c->pd.k0 : 0; }
 
+int grav_debug_log2d_binades(const grav_ctx* c) { return c ? c->pd2.nb2d : 0; }
+
 double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
     static PsiTablesHost tabs;
     static bool ready = false;
@@ -301,12 +339,28 @@ double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
 }
 
 double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0) {
-    Psi2TablesHost tabs;
-    psi2_tables_generate(&tabs, k0);
+    static std::map<int, Psi2TablesHost> cache;           // per k0
+    if (!cache.count(k0)) psi2_tables_generate(&cache[k0], k0);
+    Psi2TablesHost& tabs = cache[k0];
     Psi2TabView tb;
-    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0);
+    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0); tb.atan_base = tabs.e + kLog2N; tb.log2d = nullptr;
     const PsiColumn pc = psi_column(X, Y);
     return pc.s * psi2_fast(tb, pc, Z);
+}
+
+double grav_debug_psi2_log2d_host(double X, double Y, double Z, int k0) {
+    const int emin = -80, nb = 160;                   // the host has no shared-memory limit: tabulate 2^-80 .. 2^80
+    static std::map<int, std::vector<double2>> cache2d;      // per k0
+    std::vector<double2>& t2d = cache2d[k0];
+    if (t2d.empty()) { t2d.assign((size_t)nb * 256, double2()); psi2_log2d_generate(t2d.data(), k0, emin, nb); }
+    static std::map<int, Psi2TablesHost> cache;
+    if (!cache.count(k0)) psi2_tables_generate(&cache[k0], k0);
+    Psi2TablesHost& tabs = cache[k0];
+    Psi2TabView tb;
+    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0); tb.atan_base = tabs.e + kLog2N;
+    tb.log2d = reinterpret_cast<const char*>(t2d.data()) - ((size_t)(emin + 1023) << 12);
+    const PsiColumn pc = psi_column(X, Y);
+    return pc.s * psi2_fast_t<true>(tb, pc, Z);
 }
 
 grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {

@@ -29,6 +29,7 @@ struct Geom {
 // Launch plans fixed at context creation (deterministic reduction orders).
 struct Plan {
     // forward: grid (obs tiles, node-column chunks)
+    int log2d;             // 1: kernels use the 2-D log table (psi2.cuh LOG2D)
     int fwd_tpb, fwd_obs_per_thread, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
     // adjoint: grid (node-thread blocks, station chunks)
     int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;

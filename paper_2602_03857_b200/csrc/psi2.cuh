@@ -81,7 +81,44 @@ struct Psi2TabView {
     const double2* base;   // already offset by the thread's copy; entry i at base[i << shift]
     int shift;
     Psi2Consts k;
+    const double2* atan_base;   // first atan entry of the thread's copy; entry j at atan_base[j << shift]
+    const char* log2d;     // LOG2D variant: single-copy table indexed by exponent AND mantissa, pre-offset so that
+                           // the entry of a sits at log2d + ((hi_word(a) & 0xfffff000) >> 8); NULL otherwise
 };
+
+// LOG2D variant (experimental, profiles/r1_log2d_experiment.md): one table over every binade the arguments can
+// reach, entry = (invc 2^-e, logc + (e - k0) ln2): no exponent extraction, no I2F, no scaling of invc, one FP64
+// instruction fewer.  The price is 4 KB of shared memory per binade and a single copy (bank conflicts when the
+// lanes of a warp look up unrelated entries).  Valid only when every argument lies in the tabulated binades; the
+// context checks that from the geometry (grav_api.cu) and otherwise keeps the 256-entry evaluator.
+constexpr int kLog2dMaxBinades = 40;          // 160 KB; arguments may span a ratio of 2^40
+inline void psi2_log2d_generate(double2* out, int k0, int emin, int nb) {
+    const long double ln2 = logl(2.0L);
+    for (int b = 0; b < nb; ++b) {
+        const int e = emin + b;                       // unbiased exponent of the argument
+        for (int i = 0; i < 256; ++i) {
+            long double centre = 1.0L + ((long double)i + 0.5L) / 256.0L;
+            double invc = (double)(1.0L / centre);
+            out[b * 256 + i].x = ldexp(invc, -e);
+            out[b * 256 + i].y = (double)(-logl((long double)invc) + (long double)(e - k0) * ln2);
+        }
+    }
+}
+GRAV_HOSTDEV double log2d_fast(const Psi2TabView& tb, double a) {
+    const unsigned m = (unsigned)hi_word(a) & 0xfffff000u;
+#ifdef __CUDA_ARCH__
+    const double2 ent = *reinterpret_cast<const double2*>(tb.log2d + __umulhi(m, 1u << 24));
+#else
+    const double2 ent = *reinterpret_cast<const double2*>(tb.log2d + (m >> 8));
+#endif
+    const double r = fma(a, ent.x, -1.0);
+    const double r2 = r * r;
+    double q = fma(r, tb.k.l5, -0.25);
+    q = fma(q, r, tb.k.l3);
+    q = fma(q, r, -0.5);
+    const double p = fma(r2, q, r);
+    return ent.y + p;
+}
 
 // ln(a / 2^k0) for 0 < a < 2^1000 (finite garbage for a == 0: reading C6, the caller multiplies it by an exact 0).
 GRAV_HOSTDEV double log2_fast(const Psi2TabView& tb, double a) {
@@ -118,7 +155,8 @@ GRAV_HOSTDEV double log2_fast(const Psi2TabView& tb, double a) {
 }
 
 // Returns s * Psi(X, Y, Z) (+ the exactly-cancelling k0 offset), s = sign(XY); col from psi_column (psi.cuh).
-GRAV_HOSTDEV double psi2_fast(const Psi2TabView& tb, const PsiColumn& col, double Z) {
+template <bool LOG2D>
+GRAV_HOSTDEV double psi2_fast_t(const Psi2TabView& tb, const PsiColumn& col, double Z) {
     // ---- R = sqrt(X^2 + Y^2 + Z^2)
     const double S = fma(Z, Z, col.Q);
     const double y0 = rsqrt_seed(S);
@@ -129,8 +167,8 @@ GRAV_HOSTDEV double psi2_fast(const Psi2TabView& tb, const PsiColumn& col, doubl
     const double res1 = fma(-g1, g1, S);
     const double R = fma(res1, h0, g1);
     // ---- logarithms
-    const double L1 = log2_fast(tb, R + col.Y);
-    const double L2 = log2_fast(tb, R + col.X);
+    const double L1 = LOG2D ? log2d_fast(tb, R + col.Y) : log2_fast(tb, R + col.Y);
+    const double L2 = LOG2D ? log2d_fast(tb, R + col.X) : log2_fast(tb, R + col.X);
     // ---- angle = atan2(|XY|, |Z| R) in [0, pi/2]
     const double n = col.nXY;
     const double az = fabs(Z);
@@ -140,7 +178,7 @@ GRAV_HOSTDEV double psi2_fast(const Psi2TabView& tb, const PsiColumn& col, doubl
     const double q0 = n * rcp_seed(sum);
     const double jm = fma(q0, (double)kAtan2K, 6755399441055744.0);   // 1.5 * 2^52: low word = round(K q0)
     const int j = lo_word(jm);
-    const double2 ent = tb.base[(kLog2N + j) << tb.shift];
+    const double2 ent = tb.atan_base[j << tb.shift];
     const double num = fma(-ent.x, sum, n);
     const double den = fma(ent.x, dif, d);
     // t = num / den = num yd / (1 - e1) = num yd (1 + e1 + e1^2 + O(2^-60)),  e1 = 1 - den yd ~ 2^-20
@@ -160,10 +198,17 @@ GRAV_HOSTDEV double psi2_fast(const Psi2TabView& tb, const PsiColumn& col, doubl
     return out;
 }
 
+GRAV_HOSTDEV double psi2_fast(const Psi2TabView& tb, const PsiColumn& col, double Z) {
+    return psi2_fast_t<false>(tb, col, Z);
+}
+
 #ifdef __CUDACC__
 struct Psi2Dev {
-    const double2* tab;   // kTab2Entries entries in global memory
+    const double2* tab;     // kTab2Entries entries in global memory
     Psi2Consts k;
+    const double2* tab2d;   // LOG2D variant: nb2d * 256 entries in global memory, or NULL when the geometry rules it out
+    int nb2d;               // binades tabulated
+    int emin2d_biased;      // biased exponent of the first binade
 };
 __device__ __forceinline__ Psi2TabView psi2_tables_to_smem(double2* s_tab, const Psi2Dev& pd) {
     for (int e = threadIdx.x; e < kTab2Entries * kRep; e += blockDim.x) s_tab[e] = pd.tab[e >> kRepShift];
@@ -172,6 +217,26 @@ __device__ __forceinline__ Psi2TabView psi2_tables_to_smem(double2* s_tab, const
     v.base = s_tab + (threadIdx.x & (kRep - 1));
     v.shift = kRepShift;
     v.k = pd.k;
+    v.atan_base = v.base + (kLog2N << kRepShift);
+    v.log2d = nullptr;
+    return v;
+}
+// LOG2D layout: [atan entries, kRep interleaved copies][2-D log table, one copy, pd.nb2d * 256 entries]
+constexpr size_t kAtan2SmemBytes = (size_t)kAtan2N * kRep * sizeof(double2);
+__device__ __forceinline__ size_t psi2_log2d_smem_entries(const Psi2Dev& pd) {
+    return (size_t)kAtan2N * kRep + (size_t)pd.nb2d * 256;
+}
+__device__ __forceinline__ Psi2TabView psi2_tables_to_smem_2d(double2* s_tab, const Psi2Dev& pd) {
+    for (int e = threadIdx.x; e < kAtan2N * kRep; e += blockDim.x) s_tab[e] = pd.tab[kLog2N + (e >> kRepShift)];
+    double2* s_2d = s_tab + kAtan2N * kRep;
+    for (int e = threadIdx.x; e < pd.nb2d * 256; e += blockDim.x) s_2d[e] = pd.tab2d[e];
+    __syncthreads();
+    Psi2TabView v;
+    v.base = nullptr;
+    v.shift = kRepShift;
+    v.k = pd.k;
+    v.atan_base = s_tab + (threadIdx.x & (kRep - 1));
+    v.log2d = reinterpret_cast<const char*>(s_2d) - ((size_t)pd.emin2d_biased << 12);
     return v;
 }
 #endif
