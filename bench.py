@@ -376,7 +376,7 @@ def run_ours(args):
 
     evals = float(Nloc) * Nn                     # node evaluations one launch of this rank processes
     dom, t_dom = ("forward_nodes", t_fwd) if t_fwd >= t_adj else ("adjoint_nodes", t_adj)
-    per_eval = FP64_INST_PER_EVAL[ctx.log2d_binades > 0]
+    per_eval = FP64_INST_PER_EVAL[ctx.log2d_default]
     inst = per_eval * evals
     achieved = inst / (t_dom * 1e-3) / 1e12
     peak_nominal = 148 * FP64_LANES_PER_SM * 1.965e9 / 1e12
@@ -389,7 +389,7 @@ def run_ours(args):
                        f"DFMA-only probe in this run: {probe_rate / 1e12:.2f} T inst/s",
         "frac_of_probe": achieved / (probe_rate / 1e12),
         "frac_at_held_clock": achieved / (148 * FP64_LANES_PER_SM * clk * 1e6 / 1e12),
-        "fp64_inst_per_eval": per_eval, "log2d_binades": ctx.log2d_binades, "evals_per_launch": evals,
+        "fp64_inst_per_eval": per_eval, "log2d_binades": ctx.log2d_binades if ctx.log2d_default else 0, "evals_per_launch": evals,
         "ms_forward": t_fwd, "ms_adjoint": t_adj,
         "pairs_per_s_forward": float(Nloc) * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": float(Nloc) * M / (t_adj * 1e-3),
     }

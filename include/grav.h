@@ -194,10 +194,13 @@ double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0);
 double grav_debug_psi2_log2d_host(double X, double Y, double Z, int k0);
 /* The global exponent offset k0 chosen for this context (2^k0 ~ survey scale). */
 int grav_debug_k0(const grav_ctx* ctx);
-/* Number of binades of the exponent-and-mantissa log table this context's kernels use, or 0 when the geometry does
- * not bound the arguments of the logarithms (a station level with or inside the mesh, or a ratio above 2^40) and the
- * kernels use the 256-entry table with explicit exponent handling instead. */
+/* Number of binades of the exponent-and-mantissa log table built for this context, or 0 when the geometry does not
+ * bound the arguments of the logarithms (a station level with or inside the mesh, or a ratio above 2^40): then the
+ * kernels use the 256-entry table with explicit exponent handling. */
 int grav_debug_log2d_binades(const grav_ctx* ctx);
+/* 1 when the default kernels of this context use that table: it exists AND the problem is large enough to amortise
+ * filling it per block (stations x nodes >= 5e7); the launch variants of grav_debug_set_tuning can force either. */
+int grav_debug_log2d_default(const grav_ctx* ctx);
 
 /* Thread-local message of the last failure on this thread ("" if none). */
 const char* grav_last_error(void);

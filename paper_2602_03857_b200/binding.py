@@ -22,7 +22,7 @@ EXPORTS = [
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
     "grav_fp64_peak_probe", "grav_fp64_mix_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host", "grav_debug_psi2_log2d_host",
-    "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_set_tuning", "grav_set_allreduce",
+    "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_log2d_default", "grav_debug_set_tuning", "grav_set_allreduce",
 ]
 
 # int fn(double* buf_dev, long long count, void* stream, void* user)   (include/grav.h: grav_allreduce_fn)
@@ -106,6 +106,8 @@ def load():
     L.grav_debug_k0.argtypes = [vp]
     L.grav_debug_log2d_binades.restype = i
     L.grav_debug_log2d_binades.argtypes = [vp]
+    L.grav_debug_log2d_default.restype = i
+    L.grav_debug_log2d_default.argtypes = [vp]
     L.grav_last_error.restype = C.c_char_p
     L.grav_last_error.argtypes = []
     _lib = L
@@ -349,6 +351,10 @@ class GravContext:
     @property
     def log2d_binades(self):
         return int(self._lib.grav_debug_log2d_binades(self._h))
+
+    @property
+    def log2d_default(self):
+        return bool(self._lib.grav_debug_log2d_default(self._h))
 
     @property
     def launches(self):

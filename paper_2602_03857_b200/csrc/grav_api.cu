@@ -265,7 +265,9 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     if (e == cudaSuccess) e = init_adjoint_kernels();
     if (e == cudaSuccess) e = init_stored_kernels();
     if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaFuncSetAttribute"); }
-    make_plan(g, c->pd2.tab2d != nullptr, c->plan);
+    // tiny problems (config 1) would pay more for filling ~100 KB of table per block than they gain: the table is
+    // built whenever the geometry admits it, but it is the default only from 5e7 evaluations per product
+    make_plan(g, c->pd2.tab2d != nullptr && (double)g.N * (double)g.Nn >= 5e7, c->plan);
     make_layout(g, c->plan, c->lay);
     *out = c;
     return GRAV_OK;
@@ -327,6 +329,8 @@ grav_status grav_debug_set_tuning(grav_ctx* c, int which, int value) {
 int grav_debug_k0(const grav_ctx* c) { return c ? c->pd.k0 : 0; }
 
 int grav_debug_log2d_binades(const grav_ctx* c) { return c ? c->pd2.nb2d : 0; }
+
+int grav_debug_log2d_default(const grav_ctx* c) { return c ? c->plan.log2d : 0; }
 
 double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
     static PsiTablesHost tabs;

@@ -86,11 +86,15 @@ struct Psi2TabView {
                            // the entry of a sits at log2d + ((hi_word(a) & 0xfffff000) >> 8); NULL otherwise
 };
 
-// LOG2D variant (experimental, profiles/r1_log2d_experiment.md): one table over every binade the arguments can
-// reach, entry = (invc 2^-e, logc + (e - k0) ln2): no exponent extraction, no I2F, no scaling of invc, one FP64
-// instruction fewer.  The price is 4 KB of shared memory per binade and a single copy (bank conflicts when the
-// lanes of a warp look up unrelated entries).  Valid only when every argument lies in the tabulated binades; the
-// context checks that from the geometry (grav_api.cu) and otherwise keeps the 256-entry evaluator.
+// LOG2D variant (shipped where admissible; profiles/r1_tail_and_variants.md): one table over every binade the
+// arguments can reach, entry = (invc 2^-e, logc + (e - k0) ln2): no exponent extraction, no I2F, no scaling of invc,
+// one FP64 instruction fewer per logarithm - 44 FP64 + 16 other instructions per evaluation instead of 46 + 23.
+// The price is 4 KB of shared memory per binade and a single copy: the lanes of a warp collide on banks (ncu: the L1
+// data stage goes from 46 % to 97 % busy in the forward kernel), yet the kernels are 9 % faster overall, also with
+// random stations; ordering the stations along a Z-curve did not reduce the collisions (tried, reverted).
+// Valid only when every argument lies in the tabulated binades: a = R + Y obeys Zmin^2 / (2 Rmax) <= a <= 2 Rmax;
+// the context checks that from the geometry (grav_api.cu) and otherwise keeps the 256-entry evaluator, whose guards
+// (reading C6) also cover Z = 0 and a = 0.
 constexpr int kLog2dMaxBinades = 40;          // 160 KB; arguments may span a ratio of 2^40
 inline void psi2_log2d_generate(double2* out, int k0, int emin, int nb) {
     const long double ln2 = logl(2.0L);
