@@ -91,7 +91,7 @@ struct Psi2TabView {
 // one FP64 instruction fewer per logarithm - 44 FP64 + 16 other instructions per evaluation instead of 46 + 23.
 // The price is 4 KB of shared memory per binade and a single copy: the lanes of a warp collide on banks (ncu: the L1
 // data stage goes from 46 % to 97 % busy in the forward kernel), yet the kernels are 9 % faster overall, also with
-// random stations; ordering the stations along a Z-curve did not reduce the collisions (tried, reverted).
+// random stations; handing the stations over in Z-curve order changes the forward time by only -0.5 %.
 // Valid only when every argument lies in the tabulated binades: a = R + Y obeys Zmin^2 / (2 Rmax) <= a <= 2 Rmax;
 // the context checks that from the geometry (grav_api.cu) and otherwise keeps the 256-entry evaluator, whose guards
 // (reading C6) also cover Z = 0 and a = 0.
