@@ -223,7 +223,7 @@ cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* part
         switch (c->tune[0]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
             default:
             case 0:   // shipped: 2-D log table when the geometry admits it (grav_api.cu), else the 256-entry table
-                if (p.log2d) e = fwd_launch_staged<512, 8, 1, 3>(c, cnode, partial, done, s);
+                if (p.log2d) e = fwd_launch_staged<512, 12, 1, 3>(c, cnode, partial, done, s);
                 else e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s);
                 break;
             case 8: e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s); break;

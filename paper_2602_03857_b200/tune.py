@@ -12,10 +12,10 @@ import torch
 
 from . import binding, workloads
 
-FORWARD = {0: "shipped: 2-D log table if the geometry admits it, else variant 8", 8: "staged z-stream, psi2, 256 thr, unroll 8", 1: "staged, psi2, unroll 4",
+FORWARD = {0: "shipped: 2-D log table, 512 thr, unroll 12, if the geometry admits it, else variant 8", 8: "staged z-stream, psi2, 256 thr, unroll 8", 1: "staged, psi2, unroll 4",
            2: "LDG z-stream, psi2, unroll 4", 3: "LDG z-stream, psi2, unroll 8",
            4: "first generation: LDG, psi, 128 thr, unroll 2", 5: "staged, psi2, 512 thr, unroll 8",
-           6: "staged, psi2 + 2-D log table (experimental), 512 thr, unroll 8", 7: "same, unroll 4"}
+           6: "staged, psi2 + 2-D log table, 512 thr, unroll 8", 7: "same, unroll 4"}
 ADJOINT = {0: "plan's KC (shipped)", 1: "psi2, 256 thr, KC 4", 2: "psi2, 256 thr, KC 5", 3: "psi2, 128 thr, KC 6",
            4: "first generation: psi, 128 thr, KC 4", 5: "psi2, 128 thr, KC 8",
            6: "psi2 + 2-D log table, 512 thr, KC 4", 7: "psi2 + 2-D log table, 256 thr, KC 8",
