@@ -224,7 +224,20 @@ def paper_shape_leg(local, matrix_free=False):
                      mode=binding.STORED_F32)
     torch.cuda.synchronize()
     t2 = time.perf_counter()
+    # fixed-work upper bound of the paper's schedule: every one of the 30 updates runs its 20 CG iterations, the
+    # model recovery and the step product (no early stop) - the adaptive run above stops as soon as an update brings
+    # no decrease, which on this ill-conditioned system depends on the last bits of G (3-9 updates observed)
+    torch.cuda.synchronize()
+    t2b = time.perf_counter()
+    dd = torch.empty(wl.N, dtype=torch.float64, device=dev)
+    for _ in range(30):
+        cg = ctx.dataspace_cg(d_obs, w, lam, 20, mode=binding.STORED_F32)
+        ctx.forward_stored(cg["m"], out=dd)
+    torch.cuda.synchronize()
+    t2c = time.perf_counter()
     res = {"workload": wl.name, "prisms": wl.M, "stations": wl.N, "g_bytes_f32": float(wl.N) * wl.M * 4,
+           "full_budget_inversion_s": t2c - t2b, "full_budget_total_s": (t1 - t0) + (t2c - t2b),
+           "full_budget_note": "G build + 30 updates x (20 CG iterations + model recovery + step product), no early stop",
            "build_s": t1 - t0, "inversion_s": t2 - t1, "total_s": t2 - t0, "outer_updates": out["n_outer"],
            "stop": out["stop"], "rel_residual": float(out["hist"][-1]), "gpu_launches": ctx.launches - l0, "lambda": lam,
            "paper_context": {"total_s_1xA100_f32": 63.88, "total_s_cpu_epyc7h12": 1007.46,

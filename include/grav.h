@@ -179,7 +179,7 @@ grav_status grav_fp64_mix_probe(int device, int chains, int others, int warps_pe
  * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same kernels with CUDA libm (sqrt, /, atan, log).  Both are
  * tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
 grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
-/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel; value: variant index,
+/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel, 2 tabulation kernel; value: variant index,
  * 0 = default).  Every variant computes the same sums in the same order per thread. */
 grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
 /* Host-side evaluation of the variant-0 algorithm (same source, MUFU seeds emulated at 2^-20 accuracy) so that

@@ -67,6 +67,62 @@ __global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, Psi2Dev pd, T* __
     }
 }
 
+
+// Column-walking tabulation (the default): one thread owns one cell column (i, j) and walks down its nz + 1 node
+// layers for one station after another.  Everything that depends only on (station, corner column) - the four
+// PsiColumn hoists - is computed once per column instead of once per layer, the four corner evaluations of a layer
+// are independent (4 evaluations in flight per thread), and the entry of prism k is gamma (L(k+1) - L(k)) with both
+// layer values formed by the same thread: 4 evaluations per pair, no shuffles, no 64-bit index divisions.
+// Lanes are neighbouring cell columns, so a warp's stores of one layer are nz elements apart; consecutive layers
+// fill the same 32-byte sectors, which L2 merges before they reach DRAM.
+template <typename T, int TPB, int EV>   // EV 2: 256-entry log table, 3: exponent-and-mantissa log table
+__global__ void __launch_bounds__(TPB) tabulate_cols_kernel(Geom g, Psi2Dev pd, T* __restrict__ G) {
+    extern __shared__ double2 s_tab[];
+    const Psi2TabView tb = EV == 3 ? psi2_tables_to_smem_2d(s_tab, pd) : psi2_tables_to_smem(s_tab, pd);
+    const int ncc = g.nx * g.ny;
+    const int cc = blockIdx.x * TPB + threadIdx.x;
+    const int ccl = cc < ncc ? cc : ncc - 1;
+    const int i = ccl / g.ny, j = ccl - i * g.ny;
+    const double x1 = g.xn[i], x2 = g.xn[i + 1], y1 = g.yn[j], y2 = g.yn[j + 1];
+    for (long long st = blockIdx.y; st < g.N; st += gridDim.y) {
+        const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
+        const PsiColumn c11 = psi_column(x1 - xo, y1 - yo), c21 = psi_column(x2 - xo, y1 - yo),
+                        c12 = psi_column(x1 - xo, y2 - yo), c22 = psi_column(x2 - xo, y2 - yo);
+        T* __restrict__ out = G + st * g.M + (long long)ccl * g.nz;
+        double Lprev = 0.0;
+#pragma unroll 2
+        for (int c = 0; c < g.nzp; ++c) {
+            const double Z = __ldg(g.zn + c) - zo;
+            // (-1)^(da+db): (0,0)+, (1,0)-, (0,1)-, (1,1)+   (same order as layer_value)
+            double L = c11.s * psi2_fast_t<EV == 3>(tb, c11, Z);
+            L = fma(-c21.s, psi2_fast_t<EV == 3>(tb, c21, Z), L);
+            L = fma(-c12.s, psi2_fast_t<EV == 3>(tb, c12, Z), L);
+            L = fma(c22.s, psi2_fast_t<EV == 3>(tb, c22, Z), L);
+            if (c > 0 && cc < ncc) out[c - 1] = (T)(g.gamma * (L - Lprev));
+            Lprev = L;
+        }
+    }
+}
+
+template <typename T, int EV>
+static cudaError_t tabulate_cols_launch(grav_ctx* c, T* G, cudaStream_t s) {
+    constexpr int TPB = 512;
+    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 : kTab2SmemBytes;
+    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
+    static unsigned long long smem_set = 0;
+    cudaError_t e = ensure_dynamic_smem(tabulate_cols_kernel<T, TPB, EV>, smem_max, c->device, &smem_set);
+    if (e != cudaSuccess) return e;
+    const int ncc = c->g.nx * c->g.ny;
+    const unsigned gx = (unsigned)((ncc + TPB - 1) / TPB);
+    // every block fills the tables once and then loops over its stations: ~16 blocks per SM in total
+    long long gy = (148LL * 16 + gx - 1) / gx;
+    if (gy > c->g.N) gy = c->g.N;
+    if (gy > 65535) gy = 65535;
+    if (gy < 1) gy = 1;
+    tabulate_cols_kernel<T, TPB, EV><<<dim3(gx, (unsigned)gy), TPB, smem, s>>>(c->g, c->pd2, G);
+    return cudaGetLastError();
+}
+
 template <int TPB, bool FAST>
 __global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, Psi2Dev pd, const double* __restrict__ w,
                                                          double* __restrict__ diag) {
@@ -102,6 +158,64 @@ __global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, Psi2Dev pd, cons
         if (threadIdx.x == 0) diag[i] = sh[0];
         __syncthreads();
     }
+}
+
+
+// Gram diagonal with the same column walk: one block per station (grid-stride), its threads stride over the cell
+// columns, every thread accumulates G_ik^2 / w_k^2 down its columns; fixed-order block reduction.
+template <int TPB, int EV>
+__global__ void __launch_bounds__(TPB) gram_cols_kernel(Geom g, Psi2Dev pd, const double* __restrict__ w,
+                                                         double* __restrict__ diag) {
+    extern __shared__ double2 s_tab[];
+    __shared__ double sh[TPB];
+    const Psi2TabView tb = EV == 3 ? psi2_tables_to_smem_2d(s_tab, pd) : psi2_tables_to_smem(s_tab, pd);
+    const int ncc = g.nx * g.ny;
+    for (long long st = blockIdx.x; st < g.N; st += gridDim.x) {
+        const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
+        double acc = 0.0;
+        for (int cc = threadIdx.x; cc < ncc; cc += TPB) {
+            const int i = cc / g.ny, j = cc - i * g.ny;
+            const double x1 = g.xn[i] - xo, x2 = g.xn[i + 1] - xo, y1 = g.yn[j] - yo, y2 = g.yn[j + 1] - yo;
+            const PsiColumn c11 = psi_column(x1, y1), c21 = psi_column(x2, y1), c12 = psi_column(x1, y2),
+                            c22 = psi_column(x2, y2);
+            const double* __restrict__ wc = w + (long long)cc * g.nz;
+            double Lprev = 0.0;
+#pragma unroll 2
+            for (int c = 0; c < g.nzp; ++c) {
+                const double Z = __ldg(g.zn + c) - zo;
+                double L = c11.s * psi2_fast_t<EV == 3>(tb, c11, Z);
+                L = fma(-c21.s, psi2_fast_t<EV == 3>(tb, c21, Z), L);
+                L = fma(-c12.s, psi2_fast_t<EV == 3>(tb, c12, Z), L);
+                L = fma(c22.s, psi2_fast_t<EV == 3>(tb, c22, Z), L);
+                if (c > 0) {
+                    const double gv = g.gamma * (L - Lprev) / wc[c - 1];
+                    acc = fma(gv, gv, acc);
+                }
+                Lprev = L;
+            }
+        }
+        sh[threadIdx.x] = acc;
+        __syncthreads();
+        for (int k = TPB / 2; k > 0; k >>= 1) {
+            if (threadIdx.x < k) sh[threadIdx.x] += sh[threadIdx.x + k];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) diag[st] = sh[0];
+        __syncthreads();
+    }
+}
+
+template <int EV>
+static cudaError_t gram_cols_launch(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
+    constexpr int TPB = 512;
+    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 : kTab2SmemBytes;
+    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
+    static unsigned long long smem_set = 0;
+    cudaError_t e = ensure_dynamic_smem(gram_cols_kernel<TPB, EV>, smem_max, c->device, &smem_set);
+    if (e != cudaSuccess) return e;
+    const unsigned blocks = (unsigned)(c->g.N < 148 * 16 ? c->g.N : 148 * 16);
+    gram_cols_kernel<TPB, EV><<<blocks, TPB, smem, s>>>(c->g, c->pd2, w, diag);
+    return cudaGetLastError();
 }
 
 // ---- GEMV: d = G u ----------------------------------------------------------------------------------------
@@ -284,7 +398,14 @@ cudaError_t init_stored_kernels() {
 
 cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
     dim3 grid(pair_blocks(c->g, 256), (unsigned)(c->g.N < 65535 ? c->g.N : 65535));
-    if (c->psi_variant == 0) {
+    if (c->psi_variant == 0 && c->tune[2] == 0) {          // default: column-walking kernel
+        cudaError_t e;
+        if (c->plan.log2d) e = elem == 8 ? tabulate_cols_launch<double, 3>(c, (double*)G, s) : tabulate_cols_launch<float, 3>(c, (float*)G, s);
+        else e = elem == 8 ? tabulate_cols_launch<double, 2>(c, (double*)G, s) : tabulate_cols_launch<float, 2>(c, (float*)G, s);
+        c->launches++;
+        return e;
+    }
+    if (c->psi_variant == 0) {                              // tune[2] = 1: layer-per-thread kernel (A/B)
         if (elem == 8) tabulate_kernel<double, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (double*)G);
         else tabulate_kernel<float, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (float*)G);
     } else {
@@ -297,6 +418,11 @@ cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
 
 cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
     unsigned blocks = (unsigned)(c->g.N < (1 << 20) ? c->g.N : (1 << 20));
+    if (c->psi_variant == 0 && c->tune[2] == 0) {          // default: column-walking kernel
+        cudaError_t e = c->plan.log2d ? gram_cols_launch<3>(c, w, diag, s) : gram_cols_launch<2>(c, w, diag, s);
+        c->launches++;
+        return e;
+    }
     if (c->psi_variant == 0) gram_diag_kernel<256, true><<<blocks, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, w, diag);
     else gram_diag_kernel<256, false><<<blocks, 256, 0, s>>>(c->g, c->pd2, w, diag);
     c->launches++;
