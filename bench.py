@@ -34,7 +34,7 @@ UNIT = "pair evals/s"
 FP64_INST_PER_EVAL = {True: 44.0, False: 46.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 5 from the committed `ncu --set full` capture
 # (profiles/r1_ncu_full_cfg5.md); None for other configs
-NCU_DRAM_BYTES = {5: {"forward_nodes": 76.6e6, "adjoint_nodes": 453.1e6}}
+NCU_DRAM_BYTES = {5: {"forward_nodes": 76.4e6, "adjoint_nodes": 543.3e6}}
 NCU_DRAM_BYTES_STORED = {3: {"gemv": 68.745e9, "gemvt": 68.822e9}}      # profiles/r1_ncu_full_gemv_cfg3.md
 FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
 
