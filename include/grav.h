@@ -175,12 +175,13 @@ grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* 
 grav_status grav_fp64_mix_probe(int device, int chains, int others, int warps_per_smsp, int iters,
                                 double* dfma_warp_inst_per_smsp, double* ms);
 
-/* Diagnostics.  variant 0 (default): hand-built Psi evaluator (table-driven ln, reduced-argument atan, MUFU-seeded
- * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same kernels with CUDA libm (sqrt, /, atan, log).  Both are
- * tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
+/* Diagnostics.  variant 0 (default): hand-built Psi evaluator (table-driven ln, reduced-argument atan2, MUFU-seeded
+ * sqrt / reciprocal; csrc/psi2.cuh, first generation in csrc/psi.cuh); variant 1: the same tilings with CUDA libm
+ * (sqrt, /, atan, log).  Both are tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
 grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
-/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel, 2 tabulation kernel; value: variant index,
- * 0 = default).  Every variant computes the same sums in the same order per thread. */
+/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel, 2 tabulation / Gram
+ * kernels; value: variant index, 0 = default; the variants are listed in paper_2602_03857_b200/tune.py).  Every
+ * variant forms the same sums in the same order per thread; evaluator generations differ by rounding only. */
 grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
 /* Host-side evaluation of the variant-0 algorithm (same source, MUFU seeds emulated at 2^-20 accuracy) so that
  * CPU-only tests can check it: returns Psi(X,Y,Z) + (X+Y)*k0*ln2 (the offset cancels in every signed sum, see
