@@ -297,6 +297,26 @@ def test_launch_variants_against_oracle(shape):
     ctx.close()
 
 
+def test_survey_coordinates_with_large_offsets():
+    """UTM-like coordinates (x ~ 5e5 m, y ~ 4e6 m, mesh top 1,250 m below datum): the kernels work on corner-minus-station
+    differences, the exponent offset k0 and the log-table range come from distances, not from the absolute coordinates."""
+    from paper_2602_03857_b200 import binding
+    wl = workloads.make_custom(7, 6, 9, 40.0, 150, seed=21, topo_amp=60.0)
+    xn, yn, zn = wl.xn + 512345.25, wl.yn + 4187654.5, wl.zn + 1250.0
+    xo, yo, zo = wl.xo + 512345.25, wl.yo + 4187654.5, wl.zo + 1250.0
+    mesh = oracle.Mesh(xn, yn, zn)
+    rng = np.random.default_rng(8)
+    u, v = rng.standard_normal(wl.M), rng.standard_normal(wl.N)
+    ctx = binding.GravContext(xn, yn, zn, xo, yo, zo, wl.gamma, device=0)
+    assert ctx.log2d_binades > 0
+    for variant in (0, 6):                                    # 256-entry table (small problem default) and 2-D table
+        ctx.set_tuning(0, variant)
+        ctx.set_tuning(1, variant)
+        assert relmax(host(ctx.forward(dev(u))), oracle.forward(mesh, xo, yo, zo, wl.gamma, u)) <= TOL_OP
+        assert relmax(host(ctx.adjoint(dev(v))), oracle.adjoint(mesh, xo, yo, zo, wl.gamma, v)) <= TOL_OP
+    ctx.close()
+
+
 def test_log2d_admissibility():
     """The exponent-and-mantissa log table is used only when the geometry bounds R+Y, R+X inside 40 binades: stations
     above the mesh enable it; stations level with a node layer (Z = 0 occurs) or 0.1 mm above the top (ratio 4 Rmax^2 /
