@@ -435,12 +435,20 @@ def run_ours(args):
     stored = None
     if rank == 0 and world == 1 and not args.no_stored:
         sh.close()
-        stored = stored_g_leg(args.stored_config, local)
+        try:
+            stored = stored_g_leg(args.stored_config, local)
+        except Exception as ex:          # a secondary leg must never cost the headline line (e.g. not enough free HBM)
+            stored = {"error": f"{type(ex).__name__}: {ex}"[:300]}
+            torch.cuda.empty_cache()
 
     paper = None
     if rank == 0 and world == 1 and not args.no_paper_shape:
         sh.close()
-        paper = paper_shape_leg(local, args.paper_shape_matrix_free)
+        try:
+            paper = paper_shape_leg(local, args.paper_shape_matrix_free)
+        except Exception as ex:
+            paper = {"error": f"{type(ex).__name__}: {ex}"[:300]}
+            torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
