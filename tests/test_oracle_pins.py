@@ -324,3 +324,31 @@ def test_outer_loop_reduces_to_eq10_and_iterates(cfg1):
     m0 = np.arange(M, dtype=np.float64) % 7
     m1, _, hist, steps = oracle.invert(G, w, lam, oracle.dense_matvec(G, m0), mref=m0, max_outer=5)
     assert len(steps) == 0 and hist[0] <= 1e-13 and np.array_equal(m1, m0)
+
+
+def test_similarity_translation_and_axis_swap():
+    """Three invariances of Newtonian attraction that Eq. 1-3 must inherit, on seeded random prisms:
+    (a) similarity: scaling every length by s scales gz by s at fixed density (gz ~ gamma rho L) - a dropped or
+        doubled term of Psi with the wrong homogeneity, or a log whose argument carries a stray length, fails it;
+    (b) translation: shifting station and prism together changes nothing (only differences enter, reading C1);
+    (c) exchanging the roles of x and y (station and box) changes nothing: Psi is symmetric in (x, y) - a swapped
+        X ln(R+Y) / Y ln(R+X) pairing that is not symmetric fails it."""
+    rng = np.random.default_rng(42)
+    for _ in range(200):
+        c = rng.uniform(-500, 500, 3)
+        half = rng.uniform(5, 200, 3)
+        box = (c[0] - half[0], c[0] + half[0], c[1] - half[1], c[1] + half[1], 300 + c[2] - half[2] + 200,
+               300 + c[2] + half[2] + 200)
+        st = (rng.uniform(-800, 800), rng.uniform(-800, 800), -rng.uniform(1, 50))
+        g0 = oracle.prism_gz(st, box, 350.0, GAMMA)
+        assert g0 > 0
+        s = float(rng.uniform(0.01, 300.0))
+        gs = oracle.prism_gz(tuple(s * v for v in st), tuple(s * v for v in box), 350.0, GAMMA)
+        assert gs == pytest.approx(s * g0, rel=5e-10)          # the closed form's own cancellation at this geometry
+        t = rng.uniform(-1e4, 1e4, 3)
+        gt = oracle.prism_gz((st[0] + t[0], st[1] + t[1], st[2] + t[2]),
+                             (box[0] + t[0], box[1] + t[0], box[2] + t[1], box[3] + t[1], box[4] + t[2], box[5] + t[2]),
+                             350.0, GAMMA)
+        assert gt == pytest.approx(g0, rel=5e-9)
+        gx = oracle.prism_gz((st[1], st[0], st[2]), (box[2], box[3], box[0], box[1], box[4], box[5]), 350.0, GAMMA)
+        assert gx == pytest.approx(g0, rel=1e-11)
