@@ -335,6 +335,19 @@ def test_log2d_admissibility():
         g_ref = oracle.adjoint(mesh, base.xo, base.yo, zo, base.gamma, ref)
         assert relmax(host(ctx.adjoint(dev(ref))), g_ref) <= TOL_OP
         ctx.close()
+    # stations INSIDE the mesh, between two node layers (3 m below layer 2): Z changes sign down a column but never
+    # vanishes, so the table is admissible; force the 2-D variants and compare with the oracle (reading C3)
+    zo = np.full_like(base.zo, base.zn[2] + 3.0)
+    ctx = binding.GravContext(base.xn, base.yn, base.zn, base.xo, base.yo, zo, base.gamma, device=0)
+    assert ctx.log2d_binades > 0
+    ref = oracle.forward(mesh, base.xo, base.yo, zo, base.gamma, u)
+    g_ref = oracle.adjoint(mesh, base.xo, base.yo, zo, base.gamma, ref)
+    for variant in (0, 6):
+        ctx.set_tuning(0, variant)
+        ctx.set_tuning(1, variant)
+        assert relmax(host(ctx.forward(dev(u))), ref) <= TOL_OP
+        assert relmax(host(ctx.adjoint(dev(ref))), g_ref) <= TOL_OP
+    ctx.close()
 
 
 def test_allreduce_hook_placement(cfg1):
