@@ -12,7 +12,10 @@ namespace {
 template <int K, int NI>
 __global__ void mix_probe_kernel(double* out, int iters, double a, double b, int seed) {
     double x[K];
-    int iv[4] = {seed, seed * 3, seed * 5, seed * 7};
+    // thread-dependent values, so that the fillers are vector LOP3s like the integer work of the kernels (with uniform
+    // values ptxas moves them to the uniform datapath as ULOP3)
+    const int tid = (int)threadIdx.x;
+    int iv[4] = {seed + tid, seed * 3 + tid, seed * 5 - tid, seed * 7 ^ tid};
 #pragma unroll
     for (int j = 0; j < K; ++j) x[j] = a * (j + 1) + threadIdx.x;
     for (int it = 0; it < iters; ++it) {
@@ -22,7 +25,7 @@ __global__ void mix_probe_kernel(double* out, int iters, double a, double b, int
             for (int j = 0; j < K; ++j) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x[j]) : "d"(a), "d"(b));
 #pragma unroll
             for (int n = 0; n < NI; ++n)
-                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(iv[n & 3]) : "r"(seed), "r"(iv[(n + 1) & 3]));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0xe8;" : "+r"(iv[n & 3]) : "r"(tid), "r"(iv[(n + 1) & 3]));
         }
     }
     double s = 0;
