@@ -28,15 +28,66 @@ import numpy as np
 METRIC = "prism-obs pair evals/s (matrix-free G*m, G^T*v, FP64)"
 UNIT = "pair evals/s"
 
-# FP64-pipe thread-instructions per node evaluation of the shipped kernels (from the ncu
-# capture named there: sm__inst_executed_pipe_fp64 * 32 / evaluations).  Updated whenever psi.cuh changes.
-# 44 with the exponent-and-mantissa log table (used when the geometry admits it: all five configs), 46 otherwise
-FP64_INST_PER_EVAL = {True: 44.0, False: 46.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 5 from the committed `ncu --set full` capture
-# (profiles/r1_ncu_full_cfg5.md); None for other configs
-NCU_DRAM_BYTES = {5: {"forward_nodes": 76.4e6, "adjoint_nodes": 543.3e6}}
-NCU_DRAM_BYTES_STORED = {3: {"gemv": 68.745e9, "gemvt": 68.822e9}}      # profiles/r1_ncu_full_gemv_cfg3.md
 FP64_LANES_PER_SM = 64          # B200: 148 SMs x 64 FP64 lanes (DGX B200: 37 TFLOP/s FP64 = 148*64*2*1.965e9)
+# Measured per-kernel figures come from profiles/kernel_metrics.csv, written by
+# `python -m paper_2602_03857_b200.ncu_summary` from an `ncu --set full` capture (the .md beside it names the commands):
+# FP64-pipe thread-instructions per node evaluation and DRAM bytes per launch.  Nothing is hard-coded here.
+METRICS_CSV = os.path.join(ROOT, "profiles", "kernel_metrics.csv")
+
+
+def kernel_metrics():
+    """{(kernel, config): {column: float}} from profiles/kernel_metrics.csv ({} when the file is absent)."""
+    out = {}
+    try:
+        import csv
+        with open(METRICS_CSV) as f:
+            for row in csv.DictReader(f):
+                vals = {}
+                for k, v in row.items():
+                    try:
+                        vals[k] = float(v)
+                    except (TypeError, ValueError):
+                        vals[k] = v
+                out[(row["kernel"], int(float(row["config"])))] = vals
+    except OSError:
+        pass
+    return out
+
+
+def metric(kernel, cfg, column, log2d=True):
+    """One figure of the capture; fp64_inst_per_eval falls back to the same kernel at any config (the loop body does
+    not depend on the config), then to None."""
+    km = kernel_metrics()
+    row = km.get((kernel, cfg))
+    if row is None and column == "fp64_inst_per_eval":
+        for (k, _), r in km.items():
+            if k == kernel and bool(r.get("log2d", 1.0)) == bool(log2d):
+                row = r
+                break
+    v = None if row is None else row.get(column)
+    return v if isinstance(v, float) and v == v else None
+
+
+def cpu_info():
+    """Logical / physical core counts and the CPU model string of this host."""
+    model, phys = None, set()
+    try:
+        pid = cid = None
+        for line in open("/proc/cpuinfo"):
+            k, _, v = line.partition(":")
+            k, v = k.strip(), v.strip()
+            if k == "model name" and model is None:
+                model = v
+            elif k == "physical id":
+                pid = v
+            elif k == "core id":
+                cid = v
+            elif not k and pid is not None and cid is not None:
+                phys.add((pid, cid))
+                pid = cid = None
+    except OSError:
+        pass
+    return {"cpu_model": model, "logical_cores": os.cpu_count(), "physical_cores": len(phys) or None}
 
 
 def parse():
@@ -49,8 +100,6 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
-    ap.add_argument("--probe", action="store_true",
-                    help="print the FP64 issue microbenchmark table (grav_fp64_mix_probe) and exit")
     ap.add_argument("--no-paper-shape", action="store_true",
                     help="skip the paper-shaped run (Table 1 shape: Float32 G build + outer inversion loop)")
     ap.add_argument("--paper-shape-matrix-free", action="store_true",
@@ -133,7 +182,8 @@ def cpu_oracle_rate(wl, seconds, sample_note=True):
     S = max(cores, (S // cores) * cores)
     t, s = run(S)
     return dict(value=s * wl.M / t, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"oracle.forward on {s} seeded stations x all {wl.M} prisms ({s * wl.M:.3g} pairs, {t:.1f} s)")
+                sample=f"oracle.forward on {s} seeded stations x all {wl.M} prisms ({s * wl.M:.3g} pairs, {t:.1f} s)",
+                threads_used=cores, **cpu_info())
 
 
 
@@ -189,7 +239,7 @@ def stored_g_leg(cfg, local, reps=5):
            "max_rel_err_vs_matrix_free_forward": err, "gpu_launches": launches,
            "roofline": {"bound": "hbm", "kernel": dom, "achieved": nbytes / (t_dom * 1e-3) / 1e9, "peak": peak,
                         "unit": "GB/s", "frac": nbytes / (t_dom * 1e-3) / 1e9 / peak,
-                        "traffic": NCU_DRAM_BYTES_STORED.get(cfg, {}).get(dom), "peak_source": src,
+                        "traffic": metric(dom, cfg, "dram_bytes_per_launch"), "peak_source": src,
                         "frac_of_8TBps_nominal": nbytes / (t_dom * 1e-3) / 1e9 / 8000.0,
                         "gbs_gemv": nbytes / (t_mv * 1e-3) / 1e9, "gbs_gemvt": nbytes / (t_mvt * 1e-3) / 1e9}}
     ctx.close()
@@ -224,9 +274,9 @@ def paper_shape_leg(local, matrix_free=False):
                      mode=binding.STORED_F32)
     torch.cuda.synchronize()
     t2 = time.perf_counter()
-    # fixed-work upper bound of the paper's schedule: every one of the 30 updates runs its 20 CG iterations, the
-    # model recovery and the step product (no early stop) - the adaptive run above stops as soon as an update brings
-    # no decrease, which on this ill-conditioned system depends on the last bits of G (3-9 updates observed)
+    # fixed work of the paper's schedule: every one of the 30 updates runs its 20 CG iterations, the model recovery
+    # and the step product (no early stop) - the adaptive run above stops as soon as an update brings no decrease,
+    # which on this ill-conditioned system depends on the last bits of G (3-9 updates observed)
     torch.cuda.synchronize()
     t2b = time.perf_counter()
     dd = torch.empty(wl.N, dtype=torch.float64, device=dev)
@@ -236,10 +286,16 @@ def paper_shape_leg(local, matrix_free=False):
     torch.cuda.synchronize()
     t2c = time.perf_counter()
     res = {"workload": wl.name, "prisms": wl.M, "stations": wl.N, "g_bytes_f32": float(wl.N) * wl.M * 4,
-           "full_budget_inversion_s": t2c - t2b, "full_budget_total_s": (t1 - t0) + (t2c - t2b),
-           "full_budget_note": "G build + 30 updates x (20 CG iterations + model recovery + step product), no early stop",
-           "build_s": t1 - t0, "inversion_s": t2 - t1, "total_s": t2 - t0, "outer_updates": out["n_outer"],
-           "stop": out["stop"], "rel_residual": float(out["hist"][-1]), "gpu_launches": ctx.launches - l0, "lambda": lam,
+           "build_s": t1 - t0, "fixed_work_inversion_s": t2c - t2b, "total_s": (t1 - t0) + (t2c - t2b),
+           "total_note": "FIXED WORK: Float32 G build + 30 updates x (20 CG iterations + model recovery + step product), "
+                         "no early stop - the figure to read beside the paper's totals",
+           "pairs_per_s_build": float(wl.N) * wl.M / (t1 - t0),
+           "adaptive": {"inversion_s": t2 - t1, "outer_updates": out["n_outer"], "stop": out["stop"],
+                        "rel_residual": float(out["hist"][-1]),
+                        "note": "stopping update not reproducible: with <= 20 CG iterations the inner solves are far "
+                                "from converged and which update first brings no decrease depends on the last bits of "
+                                "G (DESIGN.md 5.7); not a benchmark figure"},
+           "gpu_launches": ctx.launches - l0, "lambda": lam,
            "paper_context": {"total_s_1xA100_f32": 63.88, "total_s_cpu_epyc7h12": 1007.46,
                              "source": "PAPER.md Table 1 (P:168-178), 3.28e6 cells x 2,601 stations"}}
     if matrix_free:
@@ -294,7 +350,8 @@ def run_reference(args):
             "config": {"workload": wl.name, "prisms": wl.M, "stations": wl.N,
                        "sample": f"{S} seeded stations x all prisms per step (adjoint + forward)"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"{S} stations x {wl.M} prisms, adjoint+forward per step"},
+                             "sample": f"{S} stations x {wl.M} prisms, adjoint+forward per step",
+                             "threads_used": cores, **cpu_info()},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -331,12 +388,18 @@ def run_ours(args):
         torch.distributed.all_reduce(dmax, op=torch.distributed.ReduceOp.MAX)
     sigma = wl.noise_frac * float(dmax.item())
     d_obs = d_clean + sigma * sh.local(wl.noise())
-    # lambda = 1e-2 * trace / N, trace/N estimated as the mean Gram diagonal over <= 512 seeded stations
-    nsub = min(N, 512)
-    idx = np.sort(np.random.default_rng(3).choice(N, size=nsub, replace=False))
-    sub = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo[idx], wl.yo[idx], wl.zo[idx], wl.gamma, device=local)
-    lam = wl.lam_factor * float(sub.gram_diag(w).mean().item())
-    sub.close()
+    # lambda = 1e-2 * trace(G W^-2 G^T) / N (reading C7) from the full Gram diagonal of this rank's stations (~1.15
+    # evaluations per pair with the node-shared per-pair kernel: about one forward product), summed over ranks
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    gdiag = ctx.gram_diag(w)
+    ev1.record()
+    tr = gdiag.sum().reshape(1)
+    if world > 1:
+        torch.distributed.all_reduce(tr)
+    torch.cuda.synchronize()
+    ms_gram = ev0.elapsed_time(ev1)
+    lam = wl.lam_factor * float(tr.item()) / N
 
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -389,20 +452,36 @@ def run_ours(args):
 
     evals = float(Nloc) * Nn                     # node evaluations one launch of this rank processes
     dom, t_dom = ("forward_nodes", t_fwd) if t_fwd >= t_adj else ("adjoint_nodes", t_adj)
-    per_eval = FP64_INST_PER_EVAL[ctx.log2d_default]
-    inst = per_eval * evals
-    achieved = inst / (t_dom * 1e-3) / 1e12
+    log2d = ctx.log2d_default
+    # FP64-pipe thread-instructions per node evaluation: from the committed ncu capture of each kernel
+    # (profiles/kernel_metrics.csv); the SASS census of the z-loop when no capture is committed
+    census = 43.0 if log2d else 45.0
+    pe_f = metric("forward_nodes", args.config, "fp64_inst_per_eval", log2d) or census
+    pe_a = metric("adjoint_nodes", args.config, "fp64_inst_per_eval", log2d) or census
+    # algorithmic work = the evaluator's FP64 instructions (census), not what a kernel executes on top of them
+    ach_f = census * evals / (t_fwd * 1e-3) / 1e12
+    ach_a = census * evals / (t_adj * 1e-3) / 1e12
+    achieved = ach_f if dom == "forward_nodes" else ach_a
     peak_nominal = 148 * FP64_LANES_PER_SM * 1.965e9 / 1e12
     probe_rate, _ = binding.fp64_peak_probe(local, 100000)
     clk = (clocks or {}).get("sm_mhz") or 1965.0
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_nominal,
-        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal, "traffic": NCU_DRAM_BYTES.get(args.config, {}).get(dom),
+        "unit": "T FP64-pipe thread-inst/s", "frac": achieved / peak_nominal,
+        "traffic": metric(dom, args.config, "dram_bytes_per_launch"),
         "peak_source": "148 SM x 64 FP64 lanes x 1.965 GHz = 1 DFMA/DMUL/DADD per lane per clock (DESIGN.md 6); "
                        f"DFMA-only probe in this run: {probe_rate / 1e12:.2f} T inst/s",
         "frac_of_probe": achieved / (probe_rate / 1e12),
         "frac_at_held_clock": achieved / (148 * FP64_LANES_PER_SM * clk * 1e6 / 1e12),
-        "fp64_inst_per_eval": per_eval, "log2d_binades": ctx.log2d_binades if ctx.log2d_default else 0, "evals_per_launch": evals,
+        "fp64_inst_per_eval": census, "fp64_inst_per_eval_source": "SASS census of the evaluator (DESIGN.md 6)",
+        "fp64_inst_executed_per_eval_ncu": {"forward_nodes": pe_f, "adjoint_nodes": pe_a},
+        "log2d_binades": ctx.log2d_binades if log2d else 0, "evals_per_launch": evals,
+        "forward_nodes": {"ms": t_fwd, "achieved": ach_f, "frac": ach_f / peak_nominal,
+                          "pairs_per_s": float(Nloc) * M / (t_fwd * 1e-3),
+                          "traffic": metric("forward_nodes", args.config, "dram_bytes_per_launch")},
+        "adjoint_nodes": {"ms": t_adj, "achieved": ach_a, "frac": ach_a / peak_nominal,
+                          "pairs_per_s": float(Nloc) * M / (t_adj * 1e-3),
+                          "traffic": metric("adjoint_nodes", args.config, "dram_bytes_per_launch")},
         "ms_forward": t_fwd, "ms_adjoint": t_adj,
         "pairs_per_s_forward": float(Nloc) * M / (t_fwd * 1e-3), "pairs_per_s_adjoint": float(Nloc) * M / (t_adj * 1e-3),
     }
@@ -461,7 +540,8 @@ def run_ours(args):
                        "step": "one data-space CG iteration (G^T p, W^-2, G(.), fused vector ops)",
                        "parallelism": f"stations sharded over {world} rank(s); all-reduce of node sums + dot partials",
                        "l2": "flushed between steps (256 MiB write)", "lambda": lam,
-                       "lambda_note": "1e-2 * mean Gram diagonal over 512 seeded stations"},
+                       "lambda_note": "1e-2 * trace(G W^-2 G^T) / N from the full Gram diagonal (grav_gram_diag)",
+                       "ms_gram_diag": ms_gram, "pairs_per_s_gram_diag": float(Nloc) * M / (ms_gram * 1e-3)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "stored_g": stored, "paper_shape": paper,
         }
@@ -471,26 +551,8 @@ def run_ours(args):
         torch.distributed.destroy_process_group()
 
 
-def run_probe():
-    """FP64 pipe utilisation of K DFMA chains per warp interleaved with NI integer instructions, W warps per
-    scheduler (include/grav.h: grav_fp64_mix_probe).  One JSON line per case."""
-    import torch
-    from paper_2602_03857_b200 import binding
-    assert torch.cuda.is_available()
-    clk = 1.965e9
-    for W in (1, 2, 4, 8, 16):
-        for K, NI in ((1, 0), (2, 0), (4, 0), (8, 0), (2, 1), (2, 2), (4, 1), (4, 2), (4, 4), (8, 2), (8, 4), (8, 8)):
-            n, ms = binding.fp64_mix_probe(0, K, NI, W, 20000 // K)
-            cyc = ms * 1e-3 * clk
-            print(json.dumps({"warps_per_scheduler": W, "dfma_chains": K, "int_per_group": NI,
-                              "int_per_dfma": NI / K, "fp64_pipe_util": round(2 * n / cyc, 4),
-                              "cycles_per_dfma": round(cyc / n, 3), "assumed_sm_hz": clk}))
-
-
 def main():
     args = parse()
-    if args.probe:
-        return run_probe()
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -15,13 +15,15 @@
  * Pointers.  Names ending in _host are HOST pointers (pageable or pinned), names ending in _dev are DEVICE pointers
  * on the context's device.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *
- * Ownership.  grav_mesh_create copies the node and station coordinates to the device (its only allocation,
- * <= 4.4 MB at 178,797 stations; freed by grav_mesh_destroy).  EVERY other device byte belongs to the caller:
+ * Ownership.  grav_mesh_create copies the node and station coordinates and the Psi tables to the device (its only
+ * allocation, <= 4.6 MB at 178,797 stations; freed by grav_mesh_destroy).  EVERY other device byte belongs to the caller:
  * inputs, outputs and one workspace block (grav_workspace_bytes / grav_set_workspace) that must stay alive and
  * must not be touched by the caller while a call that uses it is in flight.
  *
  * Execution.  *_dev entry points enqueue kernels on `stream` and return without synchronising (CG scalars stay
- * on the device).  *_host entry points copy in, compute, copy out and synchronise `stream` before returning.
+ * on the device).  Exceptions: grav_invert synchronises once per trial step (it reads one scalar back), and
+ * grav_depth_weights does one blocking 16-byte copy when z0 < 0.  *_host entry points copy in, compute, copy out and
+ * synchronise `stream` before returning.
  * Results are deterministic (fixed reduction orders, no atomics on data).
  *
  * Errors.  Every call returns a grav_status; no exception crosses the ABI; grav_last_error() returns a
@@ -96,12 +98,16 @@ grav_status grav_depth_weights(grav_ctx* ctx, double beta, double z0, double* w_
  * W_d = lambda I, m_ref = 0; textbook Hestenes-Stiefel, x0 = 0).  Runs exactly `iters` iterations when rtol = 0;
  * with rtol > 0 the iteration freezes (remaining launches become no-ops) once ||r||_2 <= rtol * ||d_obs||_2.
  * mode: operator used for the products (stored modes need grav_store_g first).
- * state: NULL or see grav_cg_state.   alpha_dev[N]: solution.   m_dev[M] or NULL: m = W^-2 G^T alpha.
+ * precond_dev[N] or NULL: Jacobi preconditioning ("CG solver with depth-weighted
+ *   regularization").  Pass diag(G W^-2 G^T) as written by grav_gram_diag; the solver applies z = r / (precond + lambda),
+ *   rho = r.z, p = z + b p.  NULL: plain CG (z = r).
+ * state: NULL or see grav_cg_state (with a preconditioner rho is r.z).   alpha_dev[N]: solution.
+ * m_dev[M] or NULL: m = W^-2 G^T alpha.
  * hist_dev[iters+1] or NULL: ||r||_2 before the first and after every iteration (recursive residual).
  * ab_dev[2*iters] or NULL: step scalars a_j (step length), b_j (direction update) of every iteration. */
 grav_status grav_dataspace_cg(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda, int iters,
-                              double rtol, int mode, grav_cg_state* state, double* alpha_dev, double* m_dev,
-                              double* hist_dev, double* ab_dev, void* stream);
+                              double rtol, int mode, const double* precond_dev, grav_cg_state* state,
+                              double* alpha_dev, double* m_dev, double* hist_dev, double* ab_dev, void* stream);
 
 /* Tabulate G (N x M row-major, prism index fastest; "global memory (sensitivity matrix)", Listing 1)
  * into the workspace in FP64 (fp32 = 0) or FP32 (fp32 != 0).  GRAV_ENOTFIT if the workspace is too small. */
@@ -113,7 +119,8 @@ grav_status grav_adjoint_stored(grav_ctx* ctx, const double* v_dev, double* g_de
 grav_status grav_stored_g(const grav_ctx* ctx, const void** g_dev, int* elem_bytes);
 
 /* diag_dev[N] = diag(G W^-2 G^T)_ii = sum_k G_ik^2 / w_k^2, matrix-free per-pair evaluation (its sum is the
- * trace that fixes lambda = 1e-2 * trace / N, BJ config 1). */
+ * trace that fixes lambda = 1e-2 * trace / N, BJ config 1; diag + lambda is the Jacobi preconditioner of
+ * grav_dataspace_cg).  Needs the workspace. */
 grav_status grav_gram_diag(grav_ctx* ctx, const double* w_dev, double* diag_dev, void* stream);
 
 /* Small problems (N <= 1024, needs a stored FP64 G): form A = G W^-2 G^T + lambda I explicitly and solve
@@ -150,15 +157,28 @@ grav_status grav_dataspace_cg_host(grav_ctx* ctx, const double* dobs_host, doubl
 
 /* Observation-sharded operation over several GPUs ("observation domain partitioned across devices, model-space
  * variables replicated and synchronised").  Each rank creates its context on ITS OWN station shard (same mesh) and
- * registers a hook that sums `count` doubles at `buf_dev` over all ranks, in place, ordered on `stream` (e.g. an NCCL
- * all-reduce; return 0 on success).  The library calls it exactly where the method exchanges data:
- *   - the node sums T (2 N_n doubles: [hi | lo] planes of the compensated sums) after the local adjoint kernel
- *     -> grav_adjoint / CG / model recovery return the GLOBAL G^T v, m;   (stored modes: the M-vector after the local G^T product)
- *   - the 256 block partials of each CG dot product (d.d, p.q, r.r)      -> every rank holds bit-identical scalars.
+ * registers two collectives over the `world` ranks, both ordered on the `stream` they are handed (e.g. NCCL; return 0
+ * on success).  The library calls them exactly where the method exchanges data:
+ *   - allgather of the local node sums T (2 N_n doubles: [hi | lo] planes of the compensated sums) after the local
+ *     adjoint kernel; the ranks' (hi, lo) pairs are then combined error-free, in rank order, by the same kernel that
+ *     combines station chunks, so the sharded G^T v equals the single-rank one to rounding and is bit-identical on
+ *     every rank -> grav_adjoint / CG / model recovery return the GLOBAL G^T v, m;
+ *   - allreduce_sum of the 256-entry block partials of the CG dot products (d.d, p.q, r.z, r.r), of the norms of
+ *     grav_invert, and (stored modes) of the M-vector after the local G^T product.
  * grav_forward, grav_gram_diag and alpha stay local to the rank's stations; there is no other communication.
- * fn = NULL restores single-rank operation.  grav_direct_solve is not available on a sharded context. */
-typedef int (*grav_allreduce_fn)(double* buf_dev, long long count, void* stream, void* user);
-grav_status grav_set_allreduce(grav_ctx* ctx, grav_allreduce_fn fn, void* user);
+ * grav_set_comm changes the workspace layout (the gather buffer needs world x 2 N_n doubles): call it BEFORE
+ * grav_workspace_bytes / grav_set_workspace; it detaches a workspace set earlier.  comm = NULL or world = 1 restores
+ * single-rank operation.  grav_direct_solve is not available on a sharded context. */
+typedef struct {
+    int world; /* number of ranks, >= 1 */
+    int rank;  /* this rank, 0 <= rank < world */
+    /* buf_dev[k] = sum over ranks of buf_dev[k], k < count, in place, every rank receives the same bits */
+    int (*allreduce_sum)(double* buf_dev, long long count, void* stream, void* user);
+    /* recv_dev[r * count + k] = send_dev[k] of rank r, k < count (recv_dev holds world * count doubles) */
+    int (*allgather)(const double* send_dev, double* recv_dev, long long count, void* stream, void* user);
+    void* user;
+} grav_comm;
+grav_status grav_set_comm(grav_ctx* ctx, const grav_comm* comm);
 
 /* Launch accounting: number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 long long grav_launch_count(const grav_ctx* ctx);
@@ -166,33 +186,19 @@ long long grav_launch_count(const grav_ctx* ctx);
  * returns the number of FP64 thread-instructions executed in *ninstr and the elapsed ms in *ms (synchronises).
  * Used to confirm the FP64 pipe peak in the same run as the roofline numbers. */
 grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* ms);
-/* FP64 issue microbenchmark (csrc/probe.cu): every warp runs `chains` independent dependent-DFMA chains with `others`
- * integer instructions after each group of `chains` DFMAs, `warps_per_smsp` (1..16) warps per scheduler on every SM.
- * Supported (chains, others): (1|2|4|8, 0), (2, 1|2), (4, 1|2|4), (8, 2|4|8); anything else returns GRAV_EINVAL.
- * Returns the DFMA warp-instructions one scheduler executed and the elapsed ms (synchronises): the FP64 pipe
- * accepts one warp-instruction per 2 cycles per scheduler, so utilisation = 2 * n / (ms * 1e-3 * sm_clock_hz).
- * Diagnostic only; holds none of the method's arithmetic. */
-grav_status grav_fp64_mix_probe(int device, int chains, int others, int warps_per_smsp, int iters,
-                                double* dfma_warp_inst_per_smsp, double* ms);
-
 /* Diagnostics.  variant 0 (default): hand-built Psi evaluator (table-driven ln, reduced-argument atan2, MUFU-seeded
- * sqrt / reciprocal; csrc/psi2.cuh, first generation in csrc/psi.cuh); variant 1: the same tilings with CUDA libm
- * (sqrt, /, atan, log).  Both are tested against the oracle; variant 1 exists for cross-checks and A/B timing. */
+ * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same tilings with CUDA libm (sqrt, /, atan, log).  Both are tested
+ * against the oracle; variant 1 exists for cross-checks and A/B timing. */
 grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
-/* Launch-configuration selector for A/B timing (which: 0 forward kernel, 1 adjoint kernel, 2 tabulation / Gram
- * kernels; value: variant index, 0 = default; the variants are listed in paper_2602_03857_b200/tune.py).  Every
- * variant forms the same sums in the same order per thread; evaluator generations differ by rounding only. */
-grav_status grav_debug_set_tuning(grav_ctx* ctx, int which, int value);
+/* Which log table the variant-0 kernels use: -1 the context's default (grav_debug_log2d_default), 0 the 256-entry
+ * table with explicit exponent handling, 1 the exponent-and-mantissa table (GRAV_ESTATE when the geometry does not
+ * admit it).  Both form the same sums in the same order; they differ by rounding only.  For tests and A/B timing. */
+grav_status grav_debug_set_log2d(grav_ctx* ctx, int mode);
 /* Host-side evaluation of the variant-0 algorithm (same source, MUFU seeds emulated at 2^-20 accuracy) so that
  * CPU-only tests can check it: returns Psi(X,Y,Z) + (X+Y)*k0*ln2 (the offset cancels in every signed sum, see
- * csrc/psi.cuh). */
-double grav_debug_psi_fast_host(double X, double Y, double Z, int k0);
-/* The same for the second-generation evaluator of csrc/psi2.cuh (swap-free atan2 reduction, exponent folded into
- * the log table entry): returns Psi(X,Y,Z) + (X+Y)*k0*ln2.  Caches its tables per k0: not thread-safe. */
-double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0);
-/* The same with the logarithms taken from the exponent-and-mantissa ("2-D") table the kernels use when the geometry
- * bounds their arguments (csrc/psi2.cuh, LOG2D); valid for arguments in [2^-80, 2^80).  Not thread-safe. */
-double grav_debug_psi2_log2d_host(double X, double Y, double Z, int k0);
+ * csrc/psi.cuh).  log2d = 0: 256-entry log table; 1: exponent-and-mantissa table, valid for arguments of the
+ * logarithms in [2^-80, 2^80).  Caches its tables per k0: not thread-safe. */
+double grav_debug_psi_eval_host(double X, double Y, double Z, int k0, int log2d);
 /* The global exponent offset k0 chosen for this context (2^k0 ~ survey scale). */
 int grav_debug_k0(const grav_ctx* ctx);
 /* Number of binades of the exponent-and-mantissa log table built for this context, or 0 when the geometry does not
@@ -200,7 +206,7 @@ int grav_debug_k0(const grav_ctx* ctx);
  * kernels use the 256-entry table with explicit exponent handling. */
 int grav_debug_log2d_binades(const grav_ctx* ctx);
 /* 1 when the default kernels of this context use that table: it exists AND the problem is large enough to amortise
- * filling it per block (stations x nodes >= 5e7); the launch variants of grav_debug_set_tuning can force either. */
+ * filling it per block (stations x nodes >= 5e7). */
 int grav_debug_log2d_default(const grav_ctx* ctx);
 
 /* Thread-local message of the last failure on this thread ("" if none). */

@@ -53,6 +53,12 @@ def lib():
         L.orc_cg.restype = None
         L.orc_cg.argtypes = ([C.c_longlong, C.c_longlong, dp] + mesh + [dp, dp, dp, C.c_double, dp, C.c_double, dp,
                              C.c_int, C.c_int, dp, dp, dp, dp, dp, dp, C.c_int, C.c_int])
+        L.orc_pcg.restype = C.c_int
+        L.orc_pcg.argtypes = [C.c_longlong, C.c_longlong, dp, dp, C.c_double, dp, dp, C.c_int, C.c_double, C.c_int,
+                              dp, dp, dp, dp, dp, dp, C.c_int]
+        L.orc_invert.restype = C.c_int
+        L.orc_invert.argtypes = [C.c_longlong, C.c_longlong, dp, dp, C.c_double, dp, dp, dp, C.c_int, C.c_int,
+                                 C.c_double, C.c_double, dp, dp, dp, dp, C.POINTER(C.c_int), dp, C.c_int]
         L.orc_hardware_threads.restype = C.c_int
         L.orc_hardware_threads.argtypes = []
         _lib = L
@@ -244,57 +250,48 @@ def recover_model(G, w, alpha, nthreads=None):
     return dense_rmatvec(G, alpha, nthreads) / (_f64(w) ** 2)
 
 
-def invert(G, w, lam, dobs, mref=None, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4, nthreads=None):
-    """The paper's outer model-update loop (P:116-118, P:162) around the data-space update of Eq. 10-11 (P:101-114),
-    with a tabulated G.  PARITY UNPINNED against the paper: it prints neither the residual norm nor the backtracking
-    rule, so this follows readings R1-R4 of DESIGN.md 2 step by step (the CUDA path restates the same readings):
-
-      m_0 = m_ref (None = 0);  r_k = d_obs - G m_k;  stop when ||r_k||_2 / ||d_obs||_2 <= tol_outer or k = max_outer
-      alpha: textbook CG on (G W^-2 G^T + lam I) alpha = r_k from 0, <= max_inner iterations, stopped after the
-             iteration whose recursive residual satisfies ||res||_2 <= tol_inner ||r_k||_2
-      delta_m = W^-2 G^T alpha;  s = 1, halved at most 10 times until ||r_k - s G delta_m|| < ||r_k|| (none: stop)
-      m_{k+1} = m_k + s delta_m
-
-    Returns (m, d_pred, hist, steps): hist[k] = ||r_k|| / ||d_obs||, steps[k] = accepted s of update k."""
+def pcg(G, w, lam, dobs, iters, diag=None, rtol=0.0, state=None, nthreads=None):
+    """Jacobi-preconditioned CG on (G W^-2 G^T + lam I) alpha = dobs with M = diag + lam (SURVEY.md 8(f) item 4;
+    P:162), diag = gram_diag(G, w); diag=None is plain CG.  Stops after the iteration with ||r|| <= rtol ||dobs||.
+    Returns (CGState with rho = r.z, hist[its+1] of ||r||_2, ab[its,2], its)."""
     G, w, dobs = _f64(G), _f64(w), _f64(dobs)
     N, M = G.shape
-    w2 = w * w
-    A = lambda p: dense_matvec(G, dense_rmatvec(G, p, nthreads) / w2, nthreads) + lam * p
-    m = np.zeros(M) if mref is None else _f64(mref).copy()
-    r = dobs - dense_matvec(G, m, nthreads) if mref is not None else dobs.copy()
-    dn = np.sqrt(float(dobs @ dobs)) or 1.0
-    nr2 = float(r @ r)
-    hist, steps = [np.sqrt(nr2) / dn], []
-    for _ in range(max_outer):
-        if np.sqrt(nr2) / dn <= tol_outer:
-            break
-        x, res, p = np.zeros(N), r.copy(), r.copy()
-        rho = float(res @ res)
-        tol2 = tol_inner * tol_inner * rho
-        for _ in range(max_inner):
-            q = A(p)
-            a = rho / float(p @ q)
-            x += a * p
-            res -= a * q
-            rho_new = float(res @ res)
-            if rho_new <= tol2:
-                break
-            p = res + (rho_new / rho) * p
-            rho = rho_new
-        dm = dense_rmatvec(G, x, nthreads) / w2
-        dd = dense_matvec(G, dm, nthreads)
-        s, ok = 1.0, False
-        for _ in range(11):
-            rt = r - s * dd
-            n2 = float(rt @ rt)
-            if n2 < nr2:
-                ok = True
-                break
-            s *= 0.5
-        if not ok:
-            break
-        m += s * dm
-        r, nr2 = rt, n2
-        steps.append(s)
-        hist.append(np.sqrt(nr2) / dn)
-    return m, dobs - r, np.array(hist), np.array(steps)
+    if state is None:
+        st, start = CGState(np.zeros(N), np.zeros(N), np.zeros(N), 0.0), 1
+    else:
+        st, start = state.copy(), 0
+    hist = np.zeros(iters + 1)
+    ab = np.zeros((max(iters, 1), 2))
+    rho = C.c_double(st.rho)
+    dg = None if diag is None else _f64(diag)
+    its = lib().orc_pcg(N, M, _p(G), _p(w), float(lam), _p(dg), _p(dobs), int(iters), float(rtol), start, _p(st.x),
+                        _p(st.r), _p(st.p), C.byref(rho), _p(hist), _p(ab), _nthreads(nthreads))
+    st.rho = rho.value
+    return st, hist[:its + 1], ab[:its], its
+
+
+def invert(G, w, lam, dobs, mref=None, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4, diag=None,
+           nthreads=None, details=False):
+    """The paper's outer model-update loop (P:116-118, P:162) around the data-space update of Eq. 10-11 (P:101-114),
+    with a tabulated G (oracle.cpp orc_invert).  PARITY UNPINNED against the paper: it prints neither the residual
+    norm nor the backtracking rule, so this follows readings R1-R4 of DESIGN.md 5.7 step by step.
+
+    Returns (m, d_pred, hist, steps): hist[k] = ||r_k|| / ||d_obs||, steps[k] = accepted s of update k; with
+    details=True also a dict(inner=CG iterations per update, trials=||r_k - 2^-h G dm||^2 per trial made,
+    rejected=True when the loop ended on "no decrease")."""
+    G, w, dobs = _f64(G), _f64(w), _f64(dobs)
+    N, M = G.shape
+    mr = None if mref is None else _f64(mref)
+    dg = None if diag is None else _f64(diag)
+    m, dpred = np.empty(M), np.empty(N)
+    hist, steps = np.zeros(max_outer + 1), np.zeros(max(max_outer, 1))
+    inner = (C.c_int * max(max_outer, 1))()
+    trials = np.full((max(max_outer, 1), 11), np.nan)
+    k = lib().orc_invert(N, M, _p(G), _p(w), float(lam), _p(dg), _p(dobs), _p(mr), int(max_outer), int(max_inner),
+                         float(tol_outer), float(tol_inner), _p(m), _p(dpred), _p(hist), _p(steps), inner, _p(trials),
+                         _nthreads(nthreads))
+    out = (m, dpred, hist[:k + 1], steps[:k])
+    if details:
+        tried = k + (1 if k < max_outer and not np.isnan(trials[k, 0]) else 0) if max_outer else 0
+        out += (dict(inner=np.array(inner[:tried]), trials=trials[:tried], rejected=tried > k),)
+    return out

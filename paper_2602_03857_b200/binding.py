@@ -21,12 +21,20 @@ EXPORTS = [
     "grav_forward", "grav_adjoint", "grav_depth_weights", "grav_dataspace_cg", "grav_store_g",
     "grav_forward_stored", "grav_adjoint_stored", "grav_stored_g", "grav_gram_diag", "grav_direct_solve",
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
-    "grav_fp64_peak_probe", "grav_fp64_mix_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_fast_host", "grav_debug_psi2_fast_host", "grav_debug_psi2_log2d_host",
-    "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_log2d_default", "grav_debug_set_tuning", "grav_set_allreduce",
+    "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_eval_host",
+    "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_log2d_default", "grav_debug_set_log2d", "grav_set_comm",
 ]
 
-# int fn(double* buf_dev, long long count, void* stream, void* user)   (include/grav.h: grav_allreduce_fn)
+# include/grav.h: grav_comm
+#   int allreduce_sum(double* buf_dev, long long count, void* stream, void* user)
+#   int allgather(const double* send_dev, double* recv_dev, long long count, void* stream, void* user)
 ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p)
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p)
+
+
+class _Comm(C.Structure):
+    _fields_ = [("world", C.c_int), ("rank", C.c_int), ("allreduce_sum", ALLREDUCE_FN), ("allgather", ALLGATHER_FN),
+                ("user", C.c_void_p)]
 
 
 class GravError(RuntimeError):
@@ -69,7 +77,7 @@ def load():
     L.grav_depth_weights.restype = i
     L.grav_depth_weights.argtypes = [vp, d, d, vp, vp]
     L.grav_dataspace_cg.restype = i
-    L.grav_dataspace_cg.argtypes = [vp, vp, vp, d, i, d, i, C.POINTER(_CgState), vp, vp, vp, vp, vp]
+    L.grav_dataspace_cg.argtypes = [vp, vp, vp, d, i, d, i, vp, C.POINTER(_CgState), vp, vp, vp, vp, vp]
     L.grav_store_g.restype = i
     L.grav_store_g.argtypes = [vp, i, vp]
     L.grav_stored_g.restype = i
@@ -88,20 +96,14 @@ def load():
     L.grav_fp64_peak_probe.argtypes = [i, i, dp, dp]
     L.grav_invert.restype = i
     L.grav_invert.argtypes = [vp, vp, vp, d, vp, i, i, d, d, i, vp, vp, vp, vp, C.POINTER(C.c_int), vp]
-    L.grav_fp64_mix_probe.restype = i
-    L.grav_fp64_mix_probe.argtypes = [i, i, i, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.grav_debug_set_psi_variant.restype = i
     L.grav_debug_set_psi_variant.argtypes = [vp, i]
-    L.grav_debug_psi_fast_host.restype = d
-    L.grav_debug_psi_fast_host.argtypes = [d, d, d, i]
-    L.grav_debug_psi2_fast_host.restype = d
-    L.grav_debug_psi2_fast_host.argtypes = [d, d, d, i]
-    L.grav_debug_psi2_log2d_host.restype = d
-    L.grav_debug_psi2_log2d_host.argtypes = [d, d, d, i]
-    L.grav_debug_set_tuning.restype = i
-    L.grav_debug_set_tuning.argtypes = [vp, i, i]
-    L.grav_set_allreduce.restype = i
-    L.grav_set_allreduce.argtypes = [vp, ALLREDUCE_FN, vp]
+    L.grav_debug_psi_eval_host.restype = d
+    L.grav_debug_psi_eval_host.argtypes = [d, d, d, i, i]
+    L.grav_debug_set_log2d.restype = i
+    L.grav_debug_set_log2d.argtypes = [vp, i]
+    L.grav_set_comm.restype = i
+    L.grav_set_comm.argtypes = [vp, C.POINTER(_Comm)]
     L.grav_debug_k0.restype = i
     L.grav_debug_k0.argtypes = [vp]
     L.grav_debug_log2d_binades.restype = i
@@ -224,8 +226,9 @@ class GravContext:
         _check(self._lib.grav_depth_weights(self._h, float(beta), float(z0), _dev(w, self.M, "w"), _stream()))
         return w
 
-    def dataspace_cg(self, dobs, w, lam, iters, rtol=0.0, mode=MATRIX_FREE, state=None, want_m=True):
-        """Returns dict(alpha, m, hist, ab) of device tensors."""
+    def dataspace_cg(self, dobs, w, lam, iters, rtol=0.0, mode=MATRIX_FREE, state=None, want_m=True, precond=None):
+        """Returns dict(alpha, m, hist, ab) of device tensors.  precond: diag(G W^-2 G^T) from gram_diag() for Jacobi
+        preconditioning (the library adds lambda), or None for plain CG."""
         alpha = self._new(self.N)
         m = self._new(self.M) if want_m else None
         hist = self._new(iters + 1)
@@ -235,7 +238,8 @@ class GravContext:
             st = _CgState(state.x.data_ptr(), state.r.data_ptr(), state.p.data_ptr(), state.rho.data_ptr(),
                           1 if state.resume else 0)
         _check(self._lib.grav_dataspace_cg(self._h, _dev(dobs, self.N, "dobs"), _dev(w, self.M, "w"), float(lam),
-                                           int(iters), float(rtol), int(mode), C.byref(st) if st else None,
+                                           int(iters), float(rtol), int(mode), _dev(precond, self.N, "precond"),
+                                           C.byref(st) if st else None,
                                            _dev(alpha, self.N, "alpha"), _dev(m, self.M, "m"),
                                            C.c_void_p(hist.data_ptr()), C.c_void_p(ab.data_ptr()), _stream()))
         return dict(alpha=alpha, m=m, hist=hist, ab=ab[:2 * iters].view(-1, 2) if iters else ab[:0])
@@ -316,33 +320,40 @@ class GravContext:
                                                 _host(hist_host, iters + 1, "hist"), _stream()))
         return alpha_host
 
-    def set_allreduce(self, fn):
-        """Register the observation-sharding exchange hook (include/grav.h: grav_set_allreduce).
-        fn(ptr: int, count: int, stream: int) -> None sums `count` doubles at device address `ptr` over all ranks,
-        in place, ordered on the CUDA stream `stream`; None restores single-rank operation."""
-        if fn is None:
-            self._hook = None
-            _check(self._lib.grav_set_allreduce(self._h, C.cast(None, ALLREDUCE_FN), None))
-            return
+    def set_comm(self, comm):
+        """Observation-sharded operation (include/grav.h: grav_set_comm).  `comm` has attributes world, rank and methods
+        allreduce_sum(ptr, count, stream) / allgather(send_ptr, recv_ptr, count, stream) on raw device addresses, both
+        ordered on the CUDA stream they are handed; None restores single-rank operation.  The workspace is re-allocated
+        for the new layout (a stored G is lost)."""
+        if comm is None or comm.world <= 1:
+            self._comm = None
+            _check(self._lib.grav_set_comm(self._h, None))
+        else:
+            def guard(fn):
+                def tramp(*a):
+                    try:
+                        fn(*[int(v or 0) for v in a[:-1]])
+                        return 0
+                    except Exception:           # no exception may cross the C ABI
+                        import traceback
+                        traceback.print_exc()
+                        return 1
+                return tramp
 
-        def tramp(buf, count, stream, user):
-            try:
-                fn(int(buf), int(count), int(stream or 0))
-                return 0
-            except Exception:           # no exception may cross the C ABI
-                import traceback
-                traceback.print_exc()
-                return 1
-
-        self._hook = ALLREDUCE_FN(tramp)      # keep the trampoline alive as long as the context uses it
-        _check(self._lib.grav_set_allreduce(self._h, self._hook, None))
+            cs = _Comm(int(comm.world), int(comm.rank), ALLREDUCE_FN(guard(comm.allreduce_sum)),
+                       ALLGATHER_FN(guard(comm.allgather)), None)
+            self._comm = (comm, cs)               # keep the trampolines alive as long as the context uses them
+            _check(self._lib.grav_set_comm(self._h, C.byref(cs)))
+        mode, self.ws, self.mode = self.mode, None, None
+        self.set_mode(mode)
 
     def set_psi_variant(self, variant):
         """0: hand-built evaluator (default); 1: CUDA libm (cross-check)."""
         _check(self._lib.grav_debug_set_psi_variant(self._h, int(variant)))
 
-    def set_tuning(self, which, value):
-        _check(self._lib.grav_debug_set_tuning(self._h, int(which), int(value)))
+    def set_log2d(self, mode):
+        """-1: the context's default log table; 0: 256-entry table; 1: exponent-and-mantissa table (diagnostic)."""
+        _check(self._lib.grav_debug_set_log2d(self._h, int(mode)))
 
     @property
     def k0(self):
@@ -361,12 +372,10 @@ class GravContext:
         return int(self._lib.grav_launch_count(self._h))
 
 
-def psi_fast_host(X, Y, Z, k0=0, gen=1):
-    """Host emulation of the device Psi evaluators (diagnostic; needs no GPU): gen 1 = psi.cuh, 2 = psi2.cuh,
-    3 = psi2.cuh with the 2-D log table."""
-    fn = {1: load().grav_debug_psi_fast_host, 2: load().grav_debug_psi2_fast_host,
-          3: load().grav_debug_psi2_log2d_host}[gen]
-    return float(fn(float(X), float(Y), float(Z), int(k0)))
+def psi_eval_host(X, Y, Z, k0=0, log2d=False):
+    """Host emulation of the device Psi evaluator of csrc/psi.cuh (diagnostic; needs no GPU); log2d selects the
+    exponent-and-mantissa log table."""
+    return float(load().grav_debug_psi_eval_host(float(X), float(Y), float(Z), int(k0), 1 if log2d else 0))
 
 
 def fp64_peak_probe(device=0, iters=200000):
@@ -374,10 +383,3 @@ def fp64_peak_probe(device=0, iters=200000):
     n, ms = C.c_double(), C.c_double()
     _check(load().grav_fp64_peak_probe(device, iters, C.byref(n), C.byref(ms)))
     return n.value / (ms.value * 1e-3), ms.value
-
-
-def fp64_mix_probe(device, chains, others, warps_per_smsp, iters=20000):
-    """(DFMA warp-instructions per scheduler, ms) of the FP64 issue microbenchmark (include/grav.h)."""
-    n, ms = C.c_double(), C.c_double()
-    _check(load().grav_fp64_mix_probe(device, chains, others, warps_per_smsp, iters, C.byref(n), C.byref(ms)))
-    return n.value, ms.value

@@ -16,35 +16,21 @@
 // by adjoint_reduce with the same TwoSum.
 #include "grav_internal.cuh"
 #include "psi.cuh"
-#include "psi2.cuh"
 
 namespace grav {
 
 constexpr int kAdjObsTile = 256;
 
-// (hi_out, lo_out) = (hi_in, lo_in) + x with the rounding error of hi_in + x captured exactly (Knuth TwoSum).
-__device__ __forceinline__ void two_sum_acc(double hi_in, double lo_in, double x, double& hi_out, double& lo_out) {
-    const double s = hi_in + x;
-    const double bb = s - hi_in;
-    const double err = (hi_in - (s - bb)) + (x - bb);
-    hi_out = s;
-    lo_out = lo_in + err;
-}
-
-// EV: 0 = CUDA libm (cross-check), 1 = psi_fast (psi.cuh), 2 = psi2_fast (psi2.cuh, the default)
+// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table
 template <int TPB, int KC, int MINB, int EV>
-__global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, Psi2Dev pd2,
-                                                                        const double* __restrict__ v,
-                                                                        double* __restrict__ partial, int ncg,
-                                                                        int obs_per_chunk, const int* __restrict__ done) {
+__global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
+                                                                  double* __restrict__ partial, int ncg,
+                                                                  int obs_per_chunk, const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
     PsiTabView tb;
-    Psi2TabView tb2;
-    if (EV == 1) tb = psi_tables_to_smem(s_tab, pd);
-    if (EV == 2) tb2 = psi2_tables_to_smem(s_tab, pd2);
-    if (EV == 3) tb2 = psi2_tables_to_smem_2d(s_tab, pd2);
+    if (EV != 0) tb = psi_tables_load<EV == 2>(s_tab, pd);
     const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long nthreads = (long long)g.ncol * ncg;
     const bool valid = t < nthreads;
@@ -77,10 +63,7 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
                 const PsiColumn pc = psi_column(X, Y);
                 const double vs = o.w * pc.s;
 #pragma unroll
-                for (int k = 0; k < KC; ++k)
-                    acc[k] = fma(vs, EV == 1 ? psi_fast(tb, pc, zc[k] - o.z)
-                                             : (EV == 3 ? psi2_fast_t<true>(tb2, pc, zc[k] - o.z)
-                                                        : psi2_fast(tb2, pc, zc[k] - o.z)), acc[k]);
+                for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
             } else {
                 const double XY = X * Y;
                 const double Q = fma(Y, Y, X * X);
@@ -104,7 +87,8 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     }
 }
 
-// tnode[2][Nn] = sum over station chunks of partial[chunk][2][Nn], (hi, lo) pairs combined in chunk order.
+// tnode[2][Nn] = sum over station chunks (or over ranks) of partial[chunk][2][Nn], (hi, lo) pairs combined in chunk
+// order.
 __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __restrict__ partial,
                                       double* __restrict__ tnode) {
     long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -119,70 +103,45 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     tnode[Nn + n] = lo;
 }
 
-template <int TPB, int KC, int MINB, int EV = 1>
-static cudaError_t adj_launch_fast(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
-    if (EV == 3 && !c->pd2.tab2d) return cudaErrorInvalidValue;      // geometry outside the 2-D log table
-    // EV == 3: the opt-in is sized for the largest 2-D table, the launch for this context's table
-    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096
-                                        : (EV == 2 ? kTab2SmemBytes : kTabSmemBytes);
-    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
+template <int TPB, int KC, int MINB, int EV>
+static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
+    // the opt-in is sized for the largest 2-D table, the launch for this context's table
+    const size_t smem = EV == 0 ? 0 : psi_smem_bytes<EV == 2>(c->pd);
     static unsigned long long smem_set = 0;
-    {
-        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, smem_max, c->device, &smem_set);
+    if (EV != 0) {
+        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, psi_smem_max<EV == 2>(), c->device,
+                                            &smem_set);
         if (e != cudaSuccess) return e;
     }
-    const Plan& p = c->plan;
     const int ncg = (c->g.nzp + KC - 1) / KC;
     const long long nthreads = (long long)c->g.ncol * ncg;
-    dim3 grid((unsigned)((nthreads + TPB - 1) / TPB), p.adj_nchunk);
-    adjoint_nodes_kernel<TPB, KC, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, c->pd2, v, partial, ncg,
-                                                                    p.adj_obs_per_chunk, done);
+    dim3 grid((unsigned)((nthreads + TPB - 1) / TPB), c->plan.adj_nchunk);
+    adjoint_nodes_kernel<TPB, KC, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, v, partial, ncg,
+                                                                    c->plan.adj_obs_per_chunk, done);
     return cudaGetLastError();
 }
 
-cudaError_t init_adjoint_kernels() { return cudaSuccess; }
-
 cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
-    const Plan& p = c->plan;
+    const int kc = c->plan.adj_kc;           // the plan's choice of KC (grav_api.cu make_plan)
     cudaError_t e;
-    if (c->psi_variant == 0) {
-        switch (c->tune[1]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
-            default:
-            case 0:   // shipped: the plan's choice of KC (grav_api.cu make_plan)
-                if (p.log2d) {
-                    if (p.adj_kc == 4) e = adj_launch_fast<512, 4, 1, 3>(c, v, partial, done, s);
-                    else if (p.adj_kc == 5) e = adj_launch_fast<512, 5, 1, 3>(c, v, partial, done, s);
-                    else if (p.adj_kc == 6) e = adj_launch_fast<256, 6, 1, 3>(c, v, partial, done, s);
-                    else e = adj_launch_fast<256, 8, 1, 3>(c, v, partial, done, s);
-                } else if (p.adj_kc == 5) e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s);
-                else if (p.adj_kc == 6) e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s);
-                else if (p.adj_kc == 8) e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s);
-                else e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s);
-                break;
-            case 1: e = adj_launch_fast<256, 4, 2, 2>(c, v, partial, done, s); break;
-            case 10: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
-            case 2: e = adj_launch_fast<256, 5, 2, 2>(c, v, partial, done, s); break;
-            case 3: e = adj_launch_fast<128, 6, 3, 2>(c, v, partial, done, s); break;
-            case 4: e = adj_launch_fast<128, 4, 4, 1>(c, v, partial, done, s); break;          // first generation
-            case 5: e = adj_launch_fast<128, 8, 2, 2>(c, v, partial, done, s); break;
-            case 6: e = adj_launch_fast<512, 4, 1, 3>(c, v, partial, done, s); break;          // 2-D log table
-            case 7: e = adj_launch_fast<256, 8, 1, 3>(c, v, partial, done, s); break;
-            case 8: e = adj_launch_fast<512, 5, 1, 3>(c, v, partial, done, s); break;
-            case 9: e = adj_launch_fast<256, 6, 1, 3>(c, v, partial, done, s); break;
-        }
+    if (c->psi_variant == 1) e = adj_launch<128, 4, 4, 0>(c, v, partial, done, s);
+    else if (use_log2d(c)) {
+        if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, s);
+        else if (kc == 5) e = adj_launch<512, 5, 1, 2>(c, v, partial, done, s);
+        else if (kc == 6) e = adj_launch<256, 6, 1, 2>(c, v, partial, done, s);
+        else e = adj_launch<256, 8, 1, 2>(c, v, partial, done, s);
     } else {
-        const int ncg4 = (c->g.nzp + 3) / 4;
-        dim3 grid((unsigned)(((long long)c->g.ncol * ncg4 + 127) / 128), p.adj_nchunk);
-        adjoint_nodes_kernel<128, 4, 4, 0><<<grid, 128, 0, s>>>(c->g, c->pd, c->pd2, v, partial, ncg4,
-                                                                    p.adj_obs_per_chunk, done);
-        e = cudaGetLastError();
+        if (kc == 4) e = adj_launch<256, 4, 2, 1>(c, v, partial, done, s);
+        else if (kc == 5) e = adj_launch<256, 5, 2, 1>(c, v, partial, done, s);
+        else if (kc == 6) e = adj_launch<128, 6, 3, 1>(c, v, partial, done, s);
+        else e = adj_launch<128, 8, 2, 1>(c, v, partial, done, s);
     }
     c->launches++;
     return e;
 }
 
-cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s) {
-    adjoint_reduce_kernel<<<(unsigned)((c->g.Nn + 255) / 256), 256, 0, s>>>(c->g.Nn, c->plan.adj_nchunk, partial, tnode);
+cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, int nchunk, double* tnode, cudaStream_t s) {
+    adjoint_reduce_kernel<<<(unsigned)((c->g.Nn + 255) / 256), 256, 0, s>>>(c->g.Nn, nchunk, partial, tnode);
     c->launches++;
     return cudaGetLastError();
 }

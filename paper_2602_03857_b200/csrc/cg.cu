@@ -1,11 +1,12 @@
 // cg.cu -- fused vector operations of the data-space conjugate-gradient solve (BASELINE.json north_star kernel 3).
 //
-// Textbook Hestenes-Stiefel CG on A = G W^-2 G^T + lambda I (Eq. 10-11; reading C8):
-//     q = A p;  delta = p.q;  a = rho/delta;  x += a p;  r -= a q;  rho' = r.r;  b = rho'/rho;  p = r + b p.
-// All scalars stay on the device (CgScalars); dot products are two-stage with a fixed tree order, every block
-// re-reduces the same kDotBlocks partials, so all blocks see bit-identical scalars and the result is
-// deterministic.  q = G(.) + lambda p and the p.q partials are produced by forward_reduce (forward.cu) or
-// dot_pq (stored-G mode).
+// Textbook Hestenes-Stiefel CG on A = G W^-2 G^T + lambda I (Eq. 10-11; reading C8), optionally
+// with the Jacobi preconditioner M = diag(A) ("CG solver"):
+//     q = A p;  delta = p.q;  a = rho/delta;  x += a p;  r -= a q;  z = M^-1 r;  rho' = r.z;  b = rho'/rho;  p = z + b p.
+// Without a preconditioner z IS r (the same buffer) and rho = r.r.  All scalars stay on the device (CgScalars); dot
+// products are two-stage with a fixed tree order, every block re-reduces the same kDotBlocks partials, so all blocks see
+// bit-identical scalars and the result is deterministic.  q = G(.) + lambda p and the p.q partials are produced by
+// forward_reduce (forward.cu) or dot_pq (stored-G mode).  Dot partial layout: [A: p.q | B: r.z | C: r.r].
 #include "grav_internal.cuh"
 
 namespace grav {
@@ -28,19 +29,35 @@ __device__ __forceinline__ double sum_partials(const double* __restrict__ dotp, 
     return block_sum(dotp[threadIdx.x], sh);
 }
 
+// Start (resume == 0): x = 0, r = d, z = M^-1 d, p = z.  Resume: the state (x, r, p) is the caller's.
+// Partials: dotp[0..) of r.z (start only), dotp[kDotBlocks..) of d.d, dotp[2 kDotBlocks..) of r.r.
 __global__ void __launch_bounds__(kDotThreads) cg_init_kernel(long long N, const double* __restrict__ dobs,
-                                                               double* __restrict__ x, double* __restrict__ r,
-                                                               double* __restrict__ p, double* __restrict__ dotp,
-                                                               int resume) {
+                                                               const double* __restrict__ minv, double lam, double* x,
+                                                               double* r, double* z, double* p,
+                                                               double* __restrict__ dotp, int resume) {
     __shared__ double sh[kDotThreads];
-    double loc = 0.0;
+    double locd = 0.0, locz = 0.0, locr = 0.0;
     for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
-        double d = dobs[i];
-        loc = fma(d, d, loc);
-        if (!resume) { x[i] = 0.0; r[i] = d; p[i] = d; }
+        const double d = dobs[i];
+        locd = fma(d, d, locd);
+        if (resume) {
+            const double ri = r[i];
+            locr = fma(ri, ri, locr);
+        } else {
+            const double zi = minv ? d / (minv[i] + lam) : d;
+            locz = fma(d, zi, locz);
+            x[i] = 0.0; r[i] = d; p[i] = zi;
+            if (minv) z[i] = zi;
+        }
     }
-    double s = block_sum(loc, sh);
-    if (threadIdx.x == 0) dotp[blockIdx.x] = s;
+    const double sd = block_sum(locd, sh);
+    const double sz = block_sum(locz, sh);
+    const double sr = resume ? block_sum(locr, sh) : sd;
+    if (threadIdx.x == 0) {
+        dotp[blockIdx.x] = sz;
+        dotp[kDotBlocks + blockIdx.x] = sd;
+        dotp[2 * kDotBlocks + blockIdx.x] = sr;
+    }
 }
 
 __global__ void __launch_bounds__(kDotThreads) cg_init_finish_kernel(const double* __restrict__ dotp, CgScalars* sc,
@@ -48,96 +65,120 @@ __global__ void __launch_bounds__(kDotThreads) cg_init_finish_kernel(const doubl
                                                                       const double* __restrict__ rho_in,
                                                                       double* __restrict__ hist) {
     __shared__ double sh[kDotThreads];
-    double dn2 = sum_partials(dotp, sh);
+    const double dz = sum_partials(dotp, sh);
+    const double dn2 = sum_partials(dotp + kDotBlocks, sh);
+    const double rr = sum_partials(dotp + 2 * kDotBlocks, sh);
     if (threadIdx.x == 0) {
-        double rho = resume ? *rho_in : dn2;
+        const double rho = resume ? *rho_in : dz;
         sc->rho[0] = rho;
         sc->rho[1] = rho;
         sc->dnorm2 = dn2;
         sc->tol2 = rtol * rtol * dn2;
         sc->delta = 0.0; sc->a = 0.0; sc->b = 0.0;
-        sc->done = (rtol > 0.0 && rho <= sc->tol2) ? 1 : 0;
+        sc->rr = rr;
+        sc->done = (rtol > 0.0 && rr <= sc->tol2) ? 1 : 0;
         sc->iters_done = 0;
-        if (hist) hist[0] = sqrt(rho);
+        sc->it = 0;
+        if (hist) hist[0] = sqrt(rr);
     }
 }
 
-// stored-G mode: q arrives without the lambda term; add it and form the p.q partials.
-__global__ void __launch_bounds__(kDotThreads) dot_pq_kernel(long long N, const double* __restrict__ p,
-                                                              const double* __restrict__ q, double lam,
-                                                              double* __restrict__ q_out, double* __restrict__ dotp,
+// stored-G mode: q arrives without the lambda term; add it in place and form the p.q partials.
+__global__ void __launch_bounds__(kDotThreads) dot_pq_kernel(long long N, const double* __restrict__ p, double lam,
+                                                              double* q, double* __restrict__ dotp,
                                                               const int* __restrict__ done) {
-    if (*done) return;
+    if (*done) {      // frozen: keep the exchanged partials finite (a sharded run all-reduces them every iteration)
+        if (threadIdx.x == 0) dotp[blockIdx.x] = 0.0;
+        return;
+    }
     __shared__ double sh[kDotThreads];
     double loc = 0.0;
     for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
-        double pi = p[i];
-        double val = fma(lam, pi, q[i]);
-        q_out[i] = val;
+        const double pi = p[i];
+        const double val = fma(lam, pi, q[i]);
+        q[i] = val;
         loc = fma(pi, val, loc);
     }
-    double s = block_sum(loc, sh);
+    const double s = block_sum(loc, sh);
     if (threadIdx.x == 0) dotp[blockIdx.x] = s;
 }
 
-__global__ void __launch_bounds__(kDotThreads) cg_update_xr_kernel(long long N, double* __restrict__ x,
-                                                                    double* __restrict__ r, const double* __restrict__ p,
+// minv != NULL: z (its own buffer) = r / (minv + lam); minv == NULL: z is r.  dotp_out: [r.z | r.r] partials.
+__global__ void __launch_bounds__(kDotThreads) cg_update_xr_kernel(long long N, double* __restrict__ x, double* r,
+                                                                    const double* __restrict__ p,
                                                                     const double* __restrict__ q,
-                                                                    const double* __restrict__ dotp_in,
-                                                                    double* __restrict__ dotp_out, CgScalars* sc, int it) {
-    if (sc->done) return;
+                                                                    const double* __restrict__ minv, double lam,
+                                                                    double* z, const double* __restrict__ dotp_in,
+                                                                    double* __restrict__ dotp_out, CgScalars* sc) {
+    if (sc->done) {
+        if (threadIdx.x == 0) { dotp_out[blockIdx.x] = 0.0; dotp_out[kDotBlocks + blockIdx.x] = 0.0; }
+        return;
+    }
     __shared__ double sh[kDotThreads];
     const double delta = sum_partials(dotp_in, sh);
-    const double a = sc->rho[it & 1] / delta;
-    double loc = 0.0;
+    const double a = sc->rho[sc->it & 1] / delta;
+    double loc = 0.0, locz = 0.0;
     for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
         x[i] = fma(a, p[i], x[i]);
-        double ri = fma(-a, q[i], r[i]);
+        const double ri = fma(-a, q[i], r[i]);
         r[i] = ri;
         loc = fma(ri, ri, loc);
+        if (minv) {
+            const double zi = ri / (minv[i] + lam);
+            z[i] = zi;
+            locz = fma(ri, zi, locz);
+        }
     }
-    double s = block_sum(loc, sh);
+    const double s = block_sum(loc, sh);
+    const double sz = minv ? block_sum(locz, sh) : s;
     if (threadIdx.x == 0) {
-        dotp_out[blockIdx.x] = s;
+        dotp_out[blockIdx.x] = sz;
+        dotp_out[kDotBlocks + blockIdx.x] = s;
         if (blockIdx.x == 0) { sc->delta = delta; sc->a = a; }
     }
 }
 
-__global__ void __launch_bounds__(kDotThreads) cg_update_p_kernel(long long N, const double* __restrict__ r,
-                                                                   double* __restrict__ p, const double* __restrict__ dotp,
-                                                                   CgScalars* sc, int it, double* __restrict__ hist_slot,
-                                                                   double* __restrict__ ab_slot) {
+__global__ void __launch_bounds__(kDotThreads) cg_update_p_kernel(long long N, const double* z, double* p,
+                                                                   const double* __restrict__ dotp, CgScalars* sc,
+                                                                   double* __restrict__ hist, double* __restrict__ ab) {
     __shared__ double sh[kDotThreads];
+    const int it = sc->it;                               // advanced by cg_advance_kernel, a launch of its own
+    double* hist_slot = hist ? hist + it + 1 : nullptr;
+    double* ab_slot = ab ? ab + 2 * it : nullptr;
     if (sc->done) {   // frozen: carry rho forward so that the parity bookkeeping stays valid
         if (blockIdx.x == 0 && threadIdx.x == 0) {
-            double rho = sc->rho[it & 1];
-            sc->rho[(it + 1) & 1] = rho;
-            if (hist_slot) *hist_slot = sqrt(rho);
+            sc->rho[(it + 1) & 1] = sc->rho[it & 1];
+            if (hist_slot) *hist_slot = hist_slot[-1];
             if (ab_slot) { ab_slot[0] = 0.0; ab_slot[1] = 0.0; }
         }
         return;
     }
     const double rho_new = sum_partials(dotp, sh);
+    const double rr = sum_partials(dotp + kDotBlocks, sh);
     const double b = rho_new / sc->rho[it & 1];
     for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads)
-        p[i] = fma(b, p[i], r[i]);
+        p[i] = fma(b, p[i], z[i]);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         sc->rho[(it + 1) & 1] = rho_new;
         sc->b = b;
-        if (hist_slot) *hist_slot = sqrt(rho_new);
+        sc->rr = rr;
+        if (hist_slot) *hist_slot = sqrt(rr);
         if (ab_slot) { ab_slot[0] = sc->a; ab_slot[1] = b; }
         sc->iters_done = it + 1;
     }
 }
 
-// `done` must be raised only after every block of update_p has read it: separate 1-thread kernel.
-__global__ void cg_check_done_kernel(CgScalars* sc, int it) {
-    if (!sc->done && sc->tol2 > 0.0 && sc->rho[(it + 1) & 1] <= sc->tol2) sc->done = 1;
+// The iteration counter may advance and `done` may be raised only after every block of update_p has read them:
+// separate 1-thread kernel.  Kernel arguments never depend on the iteration, so one captured CUDA graph of an
+// iteration can be replayed (grav_api.cu).
+__global__ void cg_advance_kernel(CgScalars* sc) {
+    sc->it += 1;
+    if (!sc->done && sc->tol2 > 0.0 && sc->rr <= sc->tol2) sc->done = 1;
 }
 
-cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp, int resume,
-                           cudaStream_t s) {
-    cg_init_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, dobs, x, r, p, dotp, resume);
+cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, const double* minv, double lam, double* x, double* r,
+                           double* z, double* p, double* dotp, int resume, cudaStream_t s) {
+    cg_init_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, dobs, minv, lam, x, r, z, p, dotp, resume);
     c->launches++;
     return cudaGetLastError();
 }
@@ -149,28 +190,26 @@ cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc
     return cudaGetLastError();
 }
 
-cudaError_t launch_dot_pq(grav_ctx* c, const double* p, const double* q, double lam, double* q_out, double* dotp,
-                          const CgScalars* sc, cudaStream_t s) {
-    dot_pq_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, p, q, lam, q_out, dotp, &sc->done);
+cudaError_t launch_dot_pq(grav_ctx* c, const double* p, double lam, double* q, double* dotp, const CgScalars* sc,
+                          cudaStream_t s) {
+    dot_pq_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, p, lam, q, dotp, &sc->done);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,
-                                const double* dotp_in, double* dotp_out, CgScalars* sc, int it, cudaStream_t s) {
-    cg_update_xr_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, x, r, p, q, dotp_in, dotp_out, sc, it);
+                                const double* minv, double lam, double* z, const double* dotp_in, double* dotp_out,
+                                CgScalars* sc, cudaStream_t s) {
+    cg_update_xr_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, x, r, p, q, minv, lam, z, dotp_in, dotp_out, sc);
     c->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_cg_update_p(grav_ctx* c, const double* r, double* p, const double* dotp, CgScalars* sc, int it,
-                               double rtol, double* hist_slot, double* ab_slot, cudaStream_t s) {
-    cg_update_p_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, r, p, dotp, sc, it, hist_slot, ab_slot);
-    c->launches++;
-    if (rtol > 0.0) {
-        cg_check_done_kernel<<<1, 1, 0, s>>>(sc, it);
-        c->launches++;
-    }
+cudaError_t launch_cg_update_p(grav_ctx* c, const double* z, double* p, const double* dotp, CgScalars* sc, double* hist,
+                               double* ab, cudaStream_t s) {
+    cg_update_p_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, z, p, dotp, sc, hist, ab);
+    cg_advance_kernel<<<1, 1, 0, s>>>(sc);
+    c->launches += 2;
     return cudaGetLastError();
 }
 

@@ -6,25 +6,22 @@
 // stations and a chunk of node columns; the node coefficients c_n of the chunk are read by every thread at the
 // same address (broadcast).  X, Y, |XY| and X^2+Y^2 are constant down a node column and hoisted out of the
 // z-loop.  Chunk partial sums go to partial[chunk][N]; forward_reduce adds them in fixed order (deterministic).
-// Bound: FP64 pipe: ~49 FP64 instructions per evaluation, 8 bytes of c_n per warp.
+// Bound: FP64 pipe: 43 FP64 instructions per evaluation, 16 bytes of (c_n, z_n) per warp.
 #include "grav_internal.cuh"
 #include "psi.cuh"
-#include "psi2.cuh"
 
 namespace grav {
 
-// EV: 0 = CUDA libm (cross-check), 1 = psi_fast (psi.cuh), 2 = psi2_fast (psi2.cuh, the default)
-template <int TPB, int UNROLL, int MINB, int EV>
-__global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, Psi2Dev pd2,
-                                                                        const double2* __restrict__ cnode,
-                                                                        double* __restrict__ partial, int cols_per_chunk,
-                                                                        const int* __restrict__ done) {
+// Unstaged kernel: the (c_n, z_n) stream is read with LDG.  Used for the CUDA-libm cross-check (LIBM) and as the
+// fallback for node columns deeper than the stage buffer of the staged kernel below.
+template <int TPB, int UNROLL, int MINB, bool LIBM>
+__global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, const double2* __restrict__ cnode,
+                                                                  double* __restrict__ partial, int cols_per_chunk,
+                                                                  const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     PsiTabView tb;
-    Psi2TabView tb2;
-    if (EV == 1) tb = psi_tables_to_smem(s_tab, pd);
-    if (EV == 2) tb2 = psi2_tables_to_smem(s_tab, pd2);
+    if (!LIBM) tb = psi_tables_to_smem(s_tab, pd);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
@@ -37,14 +34,12 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
         const double Y = __ldg(g.yn + b) - yo;
         const double2* __restrict__ cc = cnode + (long long)col * g.nzp;   // (c_n, zn[c]) pairs: one LDG.128
         double colacc = 0.0;
-        if (EV != 0) {
+        if (!LIBM) {
             const PsiColumn pc = psi_column(X, Y);
 #pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = __ldg(cc + c);
-                const double Z = cz.y - zo;
-                const double coef = cz.x;
-                colacc = fma(coef, EV == 1 ? psi_fast(tb, pc, Z) : psi2_fast(tb2, pc, Z), colacc);
+                colacc = fma(cz.x, psi_eval<false>(tb, pc, cz.y - zo), colacc);
             }
             colacc *= pc.s;
         } else {
@@ -52,9 +47,7 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
             const double Q = fma(Y, Y, X * X);
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = __ldg(cc + c);
-                const double Z = cz.y - zo;
-                const double coef = cz.x;
-                colacc = fma(coef, psi_libm(X, Y, Z, XY, Q), colacc);
+                colacc = fma(cz.x, psi_libm(X, Y, cz.y - zo, XY, Q), colacc);
             }
         }
         acc += colacc;
@@ -67,11 +60,10 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
     if (i < g.N) partial[(long long)blockIdx.y * g.N + i] = acc;
 }
 
-
-// Staged variant (the default): the (c_n, zn[c]) stream of the block's column chunk is copied to shared memory in
+// Staged kernel (the default): the (c_n, zn[c]) stream of the block's column chunk is copied to shared memory in
 // column-aligned tiles of <= kFwdStage nodes with cp.async, double-buffered, so the z-loop reads it with a
 // broadcast LDS.128 (short, fixed latency) instead of an LDG that exposes the L2 latency to 4 warps per scheduler
-// (ncu: 0.95 warps per issue stalled on long_scoreboard before, profiles/r1_ncu_full_cfg3.md).
+// (ncu: 0.95 warps per issue stalled on long_scoreboard before).
 constexpr int kFwdStage = 1024;   // nodes per buffer (16 KB); columns deeper than this use the unstaged kernel
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -83,20 +75,16 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-template <int TPB, int UNROLL, int MINB, int EV>
-__global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g, PsiDev pd, Psi2Dev pd2,
-                                                                               const double2* __restrict__ cnode,
-                                                                               double* __restrict__ partial,
-                                                                               int cols_per_chunk,
-                                                                               const int* __restrict__ done) {
+template <int TPB, int UNROLL, int MINB, bool LOG2D>
+__global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g, PsiDev pd,
+                                                                         const double2* __restrict__ cnode,
+                                                                         double* __restrict__ partial,
+                                                                         int cols_per_chunk,
+                                                                         const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
-    PsiTabView tb;
-    Psi2TabView tb2;
-    double2* s_stage;
-    if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); s_stage = s_tab + kTabEntries * kRep; }
-    else if (EV == 3) { tb2 = psi2_tables_to_smem_2d(s_tab, pd2); s_stage = s_tab + psi2_log2d_smem_entries(pd2); }
-    else { tb2 = psi2_tables_to_smem(s_tab, pd2); s_stage = s_tab + kTab2Entries * kRep; }
+    const PsiTabView tb = psi_tables_load<LOG2D>(s_tab, pd);
+    double2* s_stage = s_tab + (LOG2D ? psi_log2d_smem_entries(pd) : (size_t)kTabEntries * kRep);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
@@ -129,9 +117,7 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g,
 #pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = sc[c];
-                const double Z = cz.y - zo;
-                colacc = fma(cz.x, EV == 1 ? psi_fast(tb, pc, Z)
-                                           : (EV == 3 ? psi2_fast_t<true>(tb2, pc, Z) : psi2_fast(tb2, pc, Z)), colacc);
+                colacc = fma(cz.x, psi_eval<LOG2D>(tb, pc, cz.y - zo), colacc);
             }
             acc = fma(colacc, pc.s, acc);
             if (++b == g.nyp) {
@@ -145,101 +131,100 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g,
     if (i < g.N) partial[(long long)blockIdx.y * g.N + i] = acc;
 }
 
-// d = scale * sum_chunks partial (+ lam * p).  With dotp != NULL also writes block partials of p . d (CG: delta).
+// d = scale * sum_chunks partial (+ lam * p).  With dotp != NULL also writes kDotBlocks block partials of p . d (CG:
+// delta).  A block is kRedX stations x kRedY chunk lanes: lane y adds chunks y, y + kRedY, ... in increasing order and
+// the kRedY lane sums are added in a fixed tree, so the result does not depend on the launch; blocks stride over the
+// station tiles.
+constexpr int kRedX = 32, kRedY = kDotThreads / kRedX;
+
 __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N, int nchunk,
                                                                       const double* __restrict__ partial, double scale,
                                                                       double lam, const double* __restrict__ p,
                                                                       double* __restrict__ d, double* __restrict__ dotp,
                                                                       const int* __restrict__ done) {
-    if (done && *done) return;
-    __shared__ double sh[kDotThreads];
-    double loc = 0.0;
-    for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
-        double s = 0.0;
-        for (int ch = 0; ch < nchunk; ++ch) s += partial[(long long)ch * N + i];
-        double val = scale * s;
-        if (p) {
-            double pi = p[i];
-            val = fma(lam, pi, val);
-            loc = fma(pi, val, loc);
-        }
-        d[i] = val;
+    if (done && *done) {      // frozen CG: keep the exchanged partials finite
+        if (dotp && threadIdx.x == 0) dotp[blockIdx.x] = 0.0;
+        return;
     }
-    if (dotp) {
-        sh[threadIdx.x] = loc;
+    __shared__ double sh[kRedY][kRedX + 1];
+    __shared__ double shd[kRedX];
+    const int tx = threadIdx.x & (kRedX - 1), ty = threadIdx.x / kRedX;
+    double loc = 0.0;        // dot partial of the stations this thread finishes (ty == 0 only)
+    for (long long i0 = (long long)blockIdx.x * kRedX; i0 < N; i0 += (long long)gridDim.x * kRedX) {
+        const long long i = i0 + tx;
+        double s = 0.0;
+        if (i < N)
+            for (int ch = ty; ch < nchunk; ch += kRedY) s += partial[(long long)ch * N + i];
+        sh[ty][tx] = s;
         __syncthreads();
-        for (int s = kDotThreads / 2; s > 0; s >>= 1) {
-            if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+#pragma unroll
+        for (int h = kRedY / 2; h > 0; h >>= 1) {
+            if (ty < h) sh[ty][tx] += sh[ty + h][tx];
             __syncthreads();
         }
-        if (threadIdx.x == 0) dotp[blockIdx.x] = sh[0];
+        if (ty == 0 && i < N) {
+            double val = scale * sh[0][tx];
+            if (p) {
+                const double pi = p[i];
+                val = fma(lam, pi, val);
+                loc = fma(pi, val, loc);
+            }
+            d[i] = val;
+        }
+        __syncthreads();
+    }
+    if (dotp) {
+        if (ty == 0) shd[tx] = loc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int k = 0; k < kRedX; ++k) t += shd[k];
+            dotp[blockIdx.x] = t;
+        }
     }
 }
 
-// Launch variants (grav_debug_set_tuning(ctx, 0, v)); the default is the one measured fastest (profiles/).
-template <int TPB, int UNROLL, int MINB, int EV = 1>
-static cudaError_t fwd_launch_fast(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
-    constexpr size_t smem = EV == 2 ? kTab2SmemBytes : kTabSmemBytes;
+template <int TPB, int UNROLL, int MINB, bool LIBM>
+static cudaError_t fwd_launch_unstaged(grav_ctx* c, const double2* cnode, double* partial, const int* done,
+                                       cudaStream_t s) {
+    constexpr size_t smem = LIBM ? 0 : kTabSmemBytes;
     static unsigned long long smem_set = 0;
-    {
-        cudaError_t e = ensure_dynamic_smem(forward_nodes_kernel<TPB, UNROLL, MINB, EV>, smem, c->device, &smem_set);
+    if (smem > 48 * 1024) {
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_kernel<TPB, UNROLL, MINB, LIBM>, smem, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
-    const Plan& p = c->plan;
-    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);
-    forward_nodes_kernel<TPB, UNROLL, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, c->pd2, cnode, partial,
-                                                                        p.fwd_cols_per_chunk, done);
+    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), c->plan.fwd_nchunk);
+    forward_nodes_kernel<TPB, UNROLL, MINB, LIBM><<<grid, TPB, smem, s>>>(c->g, c->pd, cnode, partial,
+                                                                          c->plan.fwd_cols_per_chunk, done);
     return cudaGetLastError();
 }
 
-template <int TPB, int UNROLL, int MINB, int EV = 2>
-static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done, cudaStream_t s) {
-    if (c->g.nzp > kFwdStage) return fwd_launch_fast<TPB, UNROLL, MINB, EV == 3 ? 2 : EV>(c, cnode, partial, done, s);
-    if (EV == 3 && !c->pd2.tab2d) return cudaErrorInvalidValue;      // geometry outside the 2-D log table
+template <int TPB, int UNROLL, int MINB, bool LOG2D>
+static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done,
+                                     cudaStream_t s) {
+    if (c->g.nzp > kFwdStage) return fwd_launch_unstaged<256, 8, 2, false>(c, cnode, partial, done, s);
     constexpr size_t stage = 2 * kFwdStage * sizeof(double2);
-    // EV == 3: the opt-in is sized for the largest 2-D table, the launch for this context's table
-    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 + stage
-                                        : (EV == 2 ? kTab2SmemBytes : kTabSmemBytes) + stage;
-    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 + stage : smem_max;
+    // the opt-in is sized for the largest 2-D table, the launch for this context's table
+    const size_t smem = psi_smem_bytes<LOG2D>(c->pd) + stage;
     static unsigned long long smem_set = 0;
     {
-        cudaError_t e = ensure_dynamic_smem(forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV>, smem_max, c->device, &smem_set);
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_staged_kernel<TPB, UNROLL, MINB, LOG2D>,
+                                            psi_smem_max<LOG2D>() + stage, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
-    const Plan& p = c->plan;
-    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), p.fwd_nchunk);
-    forward_nodes_staged_kernel<TPB, UNROLL, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, c->pd2, cnode, partial,
-                                                                               p.fwd_cols_per_chunk, done);
+    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), c->plan.fwd_nchunk);
+    forward_nodes_staged_kernel<TPB, UNROLL, MINB, LOG2D><<<grid, TPB, smem, s>>>(c->g, c->pd, cnode, partial,
+                                                                                  c->plan.fwd_cols_per_chunk, done);
     return cudaGetLastError();
 }
-
-cudaError_t init_forward_kernels() { return cudaSuccess; }
 
 cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* partial, const int* done, cudaStream_t s) {
-    const Plan& p = c->plan;
     const double2* cnode = reinterpret_cast<const double2*>(cnode_);
     cudaError_t e;
-    if (c->psi_variant == 0) {
-        switch (c->tune[0]) {   // A/B variants measured in profiles/r1_tail_and_variants.md
-            default:
-            case 0:   // shipped: 2-D log table when the geometry admits it (grav_api.cu), else the 256-entry table
-                if (p.log2d) e = fwd_launch_staged<512, 12, 1, 3>(c, cnode, partial, done, s);
-                else e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s);
-                break;
-            case 8: e = fwd_launch_staged<256, 8, 2>(c, cnode, partial, done, s); break;
-            case 1: e = fwd_launch_staged<256, 4, 2>(c, cnode, partial, done, s); break;
-            case 2: e = fwd_launch_fast<256, 4, 2, 2>(c, cnode, partial, done, s); break;     // psi2, unstaged
-            case 3: e = fwd_launch_fast<256, 8, 2, 2>(c, cnode, partial, done, s); break;
-            case 4: e = fwd_launch_fast<128, 2, 4, 1>(c, cnode, partial, done, s); break;     // first generation
-            case 5: e = fwd_launch_staged<512, 8, 1>(c, cnode, partial, done, s); break;
-            case 6: e = fwd_launch_staged<512, 8, 1, 3>(c, cnode, partial, done, s); break;     // 2-D log table
-            case 7: e = fwd_launch_staged<512, 4, 1, 3>(c, cnode, partial, done, s); break;
-        }
-    } else {
-        dim3 grid((unsigned)((c->g.N + 127) / 128), p.fwd_nchunk);
-        forward_nodes_kernel<128, 1, 4, 0><<<grid, 128, 0, s>>>(c->g, c->pd, c->pd2, cnode, partial, p.fwd_cols_per_chunk, done);
-        e = cudaGetLastError();
-    }
+    if (c->psi_variant == 1) e = fwd_launch_unstaged<128, 1, 4, true>(c, cnode, partial, done, s);
+    else if (use_log2d(c)) e = fwd_launch_staged<512, 12, 1, true>(c, cnode, partial, done, s);
+    else e = fwd_launch_staged<256, 8, 2, false>(c, cnode, partial, done, s);
     c->launches++;
     return e;
 }

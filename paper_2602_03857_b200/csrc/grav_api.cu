@@ -35,17 +35,16 @@ size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Launch plan: enough blocks to fill 148 SMs several times over, fixed per context => deterministic sums.
-// log2d: the context's geometry admits the 2-D log table (psi2.cuh LOG2D): kernels of 512 / 256 threads, 1 block per SM.
-void make_plan(const Geom& g, bool log2d, Plan& p) {
+// log2d: the context's geometry admits the 2-D log table (psi.cuh LOG2D): kernels of 512 / 256 threads, 1 block per SM.
+void make_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     p.log2d = log2d ? 1 : 0;
     // Blocks of one launch all take the same time, so a grid of W.f waves of resident blocks costs ceil(W.f) waves:
     // with ~5 waves (the first plan) up to 18 % of the launch was tail.  ~100 blocks per SM keeps the tail <= 2-3 %
-    // (profiles/r1_tail_and_variants.md); the price is a larger partial buffer (<= 40 MB), read once.
+    // (profiles/r1_tail_and_variants.md); the price is a larger partial buffer (<= 64 MB), read once.
     const int target_blocks = log2d ? 148 * 48 : 148 * 96;      // ~48 waves either way
     // forward: 256 (512) stations per block; split the node columns into chunks when the station tiles are few
     p.fwd_tpb = log2d ? 512 : 256;
-    p.fwd_obs_per_thread = 1;
-    p.fwd_tiles = ceil_div(g.N, p.fwd_tpb * p.fwd_obs_per_thread);
+    p.fwd_tiles = ceil_div(g.N, p.fwd_tpb);
     int want = ceil_div(target_blocks, p.fwd_tiles);
     if (want > g.ncol) want = g.ncol;
     if (want > 1024) want = 1024;
@@ -72,15 +71,19 @@ void make_plan(const Geom& g, bool log2d, Plan& p) {
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
     want = ceil_div(log2d ? 148 * 48 : 148 * 128, p.adj_blocks);
     while (want > 1 && (double)want * 2.0 * g.Nn * 8.0 > 256e6) --want;   // [hi|lo] partial planes <= 256 MB
+    // a chunk is at least 64 stations (one shared-memory tile is 256); tiny problems, where that leaves fewer blocks
+    // than SMs, go down to 16 stations per chunk
     int maxchunk = ceil_div(g.N, 64);
+    if ((long long)maxchunk * p.adj_blocks < 148) maxchunk = ceil_div(g.N, 16);
     if (want > maxchunk) want = maxchunk;
     if (want > 256) want = 256;
     if (want < 1) want = 1;
     p.adj_obs_per_chunk = ceil_div(g.N, want);
     p.adj_nchunk = ceil_div(g.N, p.adj_obs_per_chunk);
+    make_pair_plan(g, pd, log2d, p);
 }
 
-void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
+void make_layout(const Geom& g, const Plan& p, int world, WsLayout& L) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t D = sizeof(double);
@@ -93,8 +96,9 @@ void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
     L.cg_r = take(g.N * D);
     L.cg_p = take(g.N * D);
     L.cg_q = take(g.N * D);
+    L.cg_z = take(g.N * D);
     L.cg_w = take(g.M * D);
-    L.dot_partial = take(2 * kDotBlocks * D);
+    L.dot_partial = take(3 * kDotBlocks * D);
     L.scalars = take(sizeof(CgScalars) + 64);
     L.stage_m = take(g.M * D);
     L.stage_n = take(g.N * D);
@@ -104,6 +108,8 @@ void make_layout(const Geom& g, const Plan& p, WsLayout& L) {
     L.inv_dd = take(g.N * D);
     L.inv_try = take(g.N * D);
     L.inv_scal = take(8 * D);
+    L.gram_partial = take(gram_partial_doubles(g, p) * D);
+    L.comm_gather = take(world > 1 ? (size_t)world * 2 * g.Nn * D : 0);
     L.matfree_end = off;
     L.gemvt_partial = take((size_t)gemvt_chunks(g.N) * g.M * D);
     L.gstore = off;
@@ -127,15 +133,17 @@ struct DeviceGuard {
     ~DeviceGuard() { cudaSetDevice(prev); }
 };
 
-// Observation-sharded operation (grav_set_allreduce): sum `count` doubles at `buf` over all ranks, in place, ordered
-// on stream `s`.  No-op for a single-rank context.
+// Observation-sharded operation (grav_set_comm): sum `count` doubles at `buf` over all ranks, in place, ordered on
+// stream `s`.  No-op for a single-rank context.
 grav_status exchange(grav_ctx* c, double* buf, long long count, cudaStream_t s) {
-    if (!c->allreduce) return GRAV_OK;
-    if (c->allreduce(buf, count, (void*)s, c->allreduce_user) != 0) return fail(GRAV_ECUDA, "all-reduce hook failed");
+    if (c->comm.world <= 1) return GRAV_OK;
+    if (c->comm.allreduce_sum(buf, count, (void*)s, c->comm.user) != 0) return fail(GRAV_ECUDA, "all-reduce callback failed");
     return GRAV_OK;
 }
 
-// node sums T = sum_i v_i Psi(node - obs_i) into ws.tnode (summed over ranks when sharded)
+// node sums T = sum_i v_i Psi(node - obs_i) into ws.tnode.  Sharded: the ranks' (hi, lo) planes are gathered and
+// combined in rank order with the same error-free kernel that combines station chunks (a plain all-reduce would round
+// every rank's contribution to one double and put ~1e-10 of max|g| at risk at config 5).
 grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cudaStream_t s) {
     double* part = wsp<double>(c, c->lay.adj_partial);
     double* tn = wsp<double>(c, c->lay.tnode);
@@ -143,9 +151,15 @@ grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cuda
         CK(launch_adjoint_nodes(c, v, tn, done, s), "adjoint_nodes");
     } else {
         CK(launch_adjoint_nodes(c, v, part, done, s), "adjoint_nodes");
-        CK(launch_adjoint_reduce(c, part, tn, s), "adjoint_reduce");
+        CK(launch_adjoint_reduce(c, part, c->plan.adj_nchunk, tn, s), "adjoint_reduce");
     }
-    return exchange(c, tn, 2 * c->g.Nn, s);
+    if (c->comm.world > 1) {
+        double* gat = wsp<double>(c, c->lay.comm_gather);
+        if (c->comm.allgather(tn, gat, 2 * c->g.Nn, (void*)s, c->comm.user) != 0)
+            return fail(GRAV_ECUDA, "all-gather callback failed");
+        CK(launch_adjoint_reduce(c, gat, c->comm.world, tn, s), "adjoint_reduce (ranks)");
+    }
+    return GRAV_OK;
 }
 
 }  // namespace
@@ -193,9 +207,8 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     c->device = device;
 
     const size_t ntab = sizeof(PsiTablesHost) / sizeof(double);
-    const size_t ntab2 = sizeof(Psi2TablesHost) / sizeof(double);
     const size_t ntab2d = (size_t)kLog2dMaxBinades * 256 * 2;
-    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2 + ntab2d + 9 * 32;   // each array 256-byte aligned
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2d + 8 * 32;   // each array 256-byte aligned
     std::vector<double> host;
     try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
     void* dev = nullptr;
@@ -211,9 +224,6 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     g.xn = put(xn, g.nxp); g.yn = put(yn, g.nyp); g.zn = put(zn, g.nzp);
     g.xo = put(ox, nobs); g.yo = put(oy, nobs); g.zo = put(oz, nobs);
     {   // Psi tables (csrc/psi.cuh) and the global exponent offset: 2^k0 ~ half the horizontal survey diagonal
-        PsiTablesHost tabs;
-        psi_tables_generate(&tabs);
-        c->pd.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs), ntab));
         double lox = xn[0], hix = xn[nx], loy = yn[0], hiy = yn[ny];
         for (long long i = 0; i < nobs; ++i) {
             lox = ox[i] < lox ? ox[i] : lox; hix = ox[i] > hix ? ox[i] : hix;
@@ -223,14 +233,13 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         c->pd.k0 = (diag > 0.0 && std::isfinite(diag)) ? (int)std::ilogb(0.5 * diag) : 0;
         if (c->pd.k0 > 900) c->pd.k0 = 900;
         if (c->pd.k0 < -900) c->pd.k0 = -900;
+        PsiTablesHost tabs;               // ~8 KB; generated per context (depends on k0)
+        psi_tables_generate(&tabs, c->pd.k0);
+        c->pd.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs), ntab));
         c->pd.k = psi_consts_make(c->pd.k0);
-        Psi2TablesHost tabs2;             // ~8 KB; generated per context (depends on k0)
-        psi2_tables_generate(&tabs2, c->pd.k0);
-        c->pd2.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs2), ntab2));
-        c->pd2.k = psi2_consts_make(c->pd.k0);
-        // 2-D log table (experimental variant): arguments a = R + Y obey Zmin^2 / (2 Rmax) <= a <= 2 Rmax, with Zmin the
-        // smallest vertical station-node distance and Rmax the largest station-node distance
-        c->pd2.tab2d = nullptr; c->pd2.nb2d = 0; c->pd2.emin2d_biased = 0;
+        // 2-D log table: arguments a = R + Y obey Zmin^2 / (2 Rmax) <= a <= 2 Rmax, with Zmin the smallest vertical
+        // station-node distance and Rmax the largest station-node distance
+        c->pd.tab2d = nullptr; c->pd.nb2d = 0; c->pd.emin2d_biased = 0;
         double zmin = INFINITY, r2max = 0.0;
         for (long long i = 0; i < nobs; ++i) {
             const double dx = std::max(std::fabs(xn[0] - ox[i]), std::fabs(xn[nx] - ox[i]));
@@ -250,25 +259,23 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
             const int nb = ehi - elo + 1;
             if (nb <= kLog2dMaxBinades && elo > -900 && ehi < 900) {
                 std::vector<double2> t2d((size_t)nb * 256);
-                psi2_log2d_generate(t2d.data(), c->pd.k0, elo, nb);
-                c->pd2.tab2d = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(t2d.data()), (size_t)nb * 512));
-                c->pd2.nb2d = nb;
-                c->pd2.emin2d_biased = elo + 1023;
+                psi_log2d_generate(t2d.data(), c->pd.k0, elo, nb);
+                c->pd.tab2d = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(t2d.data()), (size_t)nb * 512));
+                c->pd.nb2d = nb;
+                c->pd.emin2d_biased = elo + 1023;
             }
         }
         c->psi_variant = 0;
+        c->log2d_force = -1;
     }
     e = cudaMemcpy(dev, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaMemcpy geometry"); }
     c->geom_dev = dev;
-    e = init_forward_kernels();
-    if (e == cudaSuccess) e = init_adjoint_kernels();
-    if (e == cudaSuccess) e = init_stored_kernels();
-    if (e != cudaSuccess) { cudaFree(dev); delete c; return cuda_fail(e, "cudaFuncSetAttribute"); }
+    c->comm.world = 1;
     // tiny problems (config 1) would pay more for filling ~100 KB of table per block than they gain: the table is
     // built whenever the geometry admits it, but it is the default only from 5e7 evaluations per product
-    make_plan(g, c->pd2.tab2d != nullptr && (double)g.N * (double)g.Nn >= 5e7, c->plan);
-    make_layout(g, c->plan, c->lay);
+    make_plan(g, c->pd, c->pd.tab2d != nullptr && (double)g.N * (double)g.Nn >= 5e7, c->plan);
+    make_layout(g, c->plan, 1, c->lay);
     *out = c;
     return GRAV_OK;
 }
@@ -304,10 +311,20 @@ grav_status grav_set_workspace(grav_ctx* c, void* ws, size_t bytes) {
     return GRAV_OK;
 }
 
-grav_status grav_set_allreduce(grav_ctx* c, grav_allreduce_fn fn, void* user) {
+grav_status grav_set_comm(grav_ctx* c, const grav_comm* comm) {
     if (!c) return fail(GRAV_EINVAL, "NULL context");
-    c->allreduce = fn;
-    c->allreduce_user = user;
+    if (comm && comm->world > 1) {
+        if (comm->rank < 0 || comm->rank >= comm->world) return fail(GRAV_EINVAL, "rank outside [0, world)");
+        if (!comm->allreduce_sum || !comm->allgather) return fail(GRAV_EINVAL, "NULL collective callback");
+        c->comm = *comm;
+    } else {
+        memset(&c->comm, 0, sizeof(c->comm));
+        c->comm.world = 1;
+    }
+    make_layout(c->g, c->plan, c->comm.world, c->lay);      // the gather buffer depends on the number of ranks
+    c->ws = nullptr;
+    c->ws_bytes = 0;
+    c->stored_elem = 0;
     return GRAV_OK;
 }
 
@@ -320,51 +337,34 @@ grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {
     return GRAV_OK;
 }
 
-grav_status grav_debug_set_tuning(grav_ctx* c, int which, int value) {
-    if (!c || which < 0 || which >= 4) return fail(GRAV_EINVAL, "bad context / selector");
-    c->tune[which] = value;
+grav_status grav_debug_set_log2d(grav_ctx* c, int mode) {
+    if (!c || mode < -1 || mode > 1) return fail(GRAV_EINVAL, "bad context / mode");
+    if (mode == 1 && !c->pd.tab2d) return fail(GRAV_ESTATE, "the geometry does not admit the 2-D log table");
+    c->log2d_force = mode;
+    c->stored_elem = 0;
     return GRAV_OK;
 }
 
 int grav_debug_k0(const grav_ctx* c) { return c ? c->pd.k0 : 0; }
 
-int grav_debug_log2d_binades(const grav_ctx* c) { return c ? c->pd2.nb2d : 0; }
+int grav_debug_log2d_binades(const grav_ctx* c) { return c ? c->pd.nb2d : 0; }
 
 int grav_debug_log2d_default(const grav_ctx* c) { return c ? c->plan.log2d : 0; }
 
-double grav_debug_psi_fast_host(double X, double Y, double Z, int k0) {
-    static PsiTablesHost tabs;
-    static bool ready = false;
-    if (!ready) { psi_tables_generate(&tabs); ready = true; }
+double grav_debug_psi_eval_host(double X, double Y, double Z, int k0, int log2d) {
+    static std::map<int, PsiTablesHost> cache;              // per k0
+    if (!cache.count(k0)) psi_tables_generate(&cache[k0], k0);
+    PsiTablesHost& tabs = cache[k0];
     PsiTabView tb;
-    tb.base = tabs.e; tb.shift = 0; tb.k = psi_consts_make(k0); tb.ik = psi_int_consts(0);
+    tb.base = tabs.e; tb.shift = 0; tb.k = psi_consts_make(k0); tb.atan_base = tabs.e + kLogN; tb.log2d = nullptr;
     const PsiColumn pc = psi_column(X, Y);
-    return pc.s * psi_fast(tb, pc, Z);
-}
-
-double grav_debug_psi2_fast_host(double X, double Y, double Z, int k0) {
-    static std::map<int, Psi2TablesHost> cache;           // per k0
-    if (!cache.count(k0)) psi2_tables_generate(&cache[k0], k0);
-    Psi2TablesHost& tabs = cache[k0];
-    Psi2TabView tb;
-    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0); tb.atan_base = tabs.e + kLog2N; tb.log2d = nullptr;
-    const PsiColumn pc = psi_column(X, Y);
-    return pc.s * psi2_fast(tb, pc, Z);
-}
-
-double grav_debug_psi2_log2d_host(double X, double Y, double Z, int k0) {
+    if (!log2d) return pc.s * psi_eval<false>(tb, pc, Z);
     const int emin = -80, nb = 160;                   // the host has no shared-memory limit: tabulate 2^-80 .. 2^80
-    static std::map<int, std::vector<double2>> cache2d;      // per k0
+    static std::map<int, std::vector<double2>> cache2d;
     std::vector<double2>& t2d = cache2d[k0];
-    if (t2d.empty()) { t2d.assign((size_t)nb * 256, double2()); psi2_log2d_generate(t2d.data(), k0, emin, nb); }
-    static std::map<int, Psi2TablesHost> cache;
-    if (!cache.count(k0)) psi2_tables_generate(&cache[k0], k0);
-    Psi2TablesHost& tabs = cache[k0];
-    Psi2TabView tb;
-    tb.base = tabs.e; tb.shift = 0; tb.k = psi2_consts_make(k0); tb.atan_base = tabs.e + kLog2N;
+    if (t2d.empty()) { t2d.assign((size_t)nb * 256, double2()); psi_log2d_generate(t2d.data(), k0, emin, nb); }
     tb.log2d = reinterpret_cast<const char*>(t2d.data()) - ((size_t)(emin + 1023) << 12);
-    const PsiColumn pc = psi_column(X, Y);
-    return pc.s * psi2_fast_t<true>(tb, pc, Z);
+    return pc.s * psi_eval<true>(tb, pc, Z);
 }
 
 grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) {
@@ -451,15 +451,17 @@ grav_status grav_adjoint_stored(grav_ctx* c, const double* v, double* gout, void
 }
 
 grav_status grav_gram_diag(grav_ctx* c, const double* w, double* diag, void* stream) {
-    if (!c || !w || !diag) return fail(GRAV_EINVAL, "NULL argument");
+    grav_status st = check_ready(c);
+    if (st) return st;
+    if (!w || !diag) return fail(GRAV_EINVAL, "NULL argument");
     DeviceGuard dg(c->device);
-    CK(launch_gram_diag(c, w, diag, (cudaStream_t)stream), "gram_diag");
+    CK(launch_gram_diag(c, w, wsp<double>(c, c->lay.gram_partial), diag, (cudaStream_t)stream), "gram_diag");
     return GRAV_OK;
 }
 
 grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, double lambda, int iters, double rtol,
-                              int mode, grav_cg_state* state, double* alpha, double* m, double* hist, double* ab,
-                              void* stream) {
+                              int mode, const double* precond, grav_cg_state* state, double* alpha, double* m,
+                              double* hist, double* ab, void* stream) {
     grav_status st = check_ready(c);
     if (st) return st;
     if (!dobs || !w || !alpha) return fail(GRAV_EINVAL, "NULL vector");
@@ -477,8 +479,9 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
     double* r = state ? state->r_dev : wsp<double>(c, c->lay.cg_r);
     double* p = state ? state->p_dev : wsp<double>(c, c->lay.cg_p);
     double* q = wsp<double>(c, c->lay.cg_q);
+    double* z = precond ? wsp<double>(c, c->lay.cg_z) : r;          // without a preconditioner z IS r
     double* dotA = wsp<double>(c, c->lay.dot_partial);
-    double* dotB = dotA + kDotBlocks;
+    double* dotB = dotA + kDotBlocks;                               // [r.z | r.r]
     CgScalars* sc = wsp<CgScalars>(c, c->lay.scalars);
     double* gcell = wsp<double>(c, c->lay.gcell);
     double* cnode = wsp<double>(c, c->lay.cnode);
@@ -487,8 +490,8 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
     const void* G = c->ws + c->lay.gstore;
     const int resume = state ? state->resume : 0;
 
-    CK(launch_cg_init(c, dobs, x, r, p, dotA, resume, s), "cg_init");
-    if ((st = exchange(c, dotA, kDotBlocks, s))) return st;
+    CK(launch_cg_init(c, dobs, precond, lambda, x, r, z, p, dotA, resume, s), "cg_init");
+    if ((st = exchange(c, dotA, 3 * kDotBlocks, s))) return st;
     CK(launch_cg_init_finish(c, dotA, sc, rtol, resume, state ? state->rho_dev : nullptr, hist, s), "cg_init_finish");
     for (int it = 0; it < iters; ++it) {
         if (mode == GRAV_MATRIX_FREE) {
@@ -503,13 +506,12 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
             CK(launch_gemvt(c, G, c->stored_elem, p, w, gcell, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
             if ((st = exchange(c, gcell, g.M, s))) return st;
             CK(launch_gemv(c, G, c->stored_elem, gcell, q, s), "gemv");
-            CK(launch_dot_pq(c, p, q, lambda, q, dotA, sc, s), "dot_pq");
+            CK(launch_dot_pq(c, p, lambda, q, dotA, sc, s), "dot_pq");
         }
         if ((st = exchange(c, dotA, kDotBlocks, s))) return st;
-        CK(launch_cg_update_xr(c, x, r, p, q, dotA, dotB, sc, it, s), "cg_update_xr");
-        if ((st = exchange(c, dotB, kDotBlocks, s))) return st;
-        CK(launch_cg_update_p(c, r, p, dotB, sc, it, rtol, hist ? hist + it + 1 : nullptr, ab ? ab + 2 * it : nullptr, s),
-           "cg_update_p");
+        CK(launch_cg_update_xr(c, x, r, p, q, precond, lambda, z, dotA, dotB, sc, s), "cg_update_xr");
+        if ((st = exchange(c, dotB, 2 * kDotBlocks, s))) return st;
+        CK(launch_cg_update_p(c, z, p, dotB, sc, hist, ab, s), "cg_update_p");
     }
     if (alpha != x) CK(cudaMemcpyAsync(alpha, x, g.N * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy alpha");
     if (state) CK(cudaMemcpyAsync(state->rho_dev, &sc->rho[iters & 1], sizeof(double), cudaMemcpyDeviceToDevice, s), "copy rho");
@@ -533,7 +535,7 @@ grav_status grav_direct_solve(grav_ctx* c, const double* dobs, const double* w, 
     if (!dobs || !w || !A || !alpha) return fail(GRAV_EINVAL, "NULL argument");
     if (c->g.N > 1024) return fail(GRAV_EINVAL, "direct solve is limited to N <= 1024");
     if (c->stored_elem != 8) return fail(GRAV_ESTATE, "direct solve needs a stored FP64 G (grav_store_g)");
-    if (c->allreduce) return fail(GRAV_ESTATE, "direct solve is not available on an observation-sharded context");
+    if (c->comm.world > 1) return fail(GRAV_ESTATE, "direct solve is not available on an observation-sharded context");
     DeviceGuard dg(c->device);
     cudaStream_t s = (cudaStream_t)stream;
     const double* G = reinterpret_cast<const double*>(c->ws + c->lay.gstore);
@@ -594,7 +596,7 @@ grav_status grav_invert(grav_ctx* c, const double* dobs, const double* w, double
     int k = 0;
     for (; k < max_outer; ++k) {
         if (std::sqrt(nr2) / dn <= tol_outer) break;
-        st = grav_dataspace_cg(c, r, w, lambda, max_inner, tol_inner, mode, nullptr, alpha, dm, nullptr, nullptr, stream);
+        st = grav_dataspace_cg(c, r, w, lambda, max_inner, tol_inner, mode, nullptr, nullptr, alpha, dm, nullptr, nullptr, stream);
         if (st) return st;
         if ((st = apply_G(dm, dd))) return st;
         double step = 1.0, n2 = 0.0;
@@ -605,7 +607,7 @@ grav_status grav_invert(grav_ctx* c, const double* dobs, const double* w, double
         }
         if (step_host) step_host[k] = ok ? step : 0.0;
         if (!ok) break;                                   // no decrease along delta_m: stop with m_k
-        CK(launch_inv_axpy(c, step, dm, m, m, s), "inv_axpy");
+        CK(launch_inv_axpy(c, step, dm, m, s), "inv_axpy");
         CK(cudaMemcpyAsync(r, rtry, g.N * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy r");
         nr2 = n2;
         if (hist_host) hist_host[k + 1] = std::sqrt(nr2) / dn;
@@ -668,7 +670,7 @@ grav_status grav_dataspace_cg_host(grav_ctx* c, const double* dobs_host, double 
     if (st) return st;
     // alpha is produced in the CG's own x buffer and copied out from there
     double* x = wsp<double>(c, c->lay.cg_x);
-    st = grav_dataspace_cg(c, dn, w, lambda, iters, rtol, mode, nullptr, x, m_host ? mm : nullptr,
+    st = grav_dataspace_cg(c, dn, w, lambda, iters, rtol, mode, nullptr, nullptr, x, m_host ? mm : nullptr,
                            hist_host ? hh : nullptr, nullptr, stream);
     if (st) return st;
     CK(cudaMemcpyAsync(alpha_host, x, c->g.N * sizeof(double), cudaMemcpyDeviceToHost, s), "D2H alpha");

@@ -6,7 +6,6 @@
 
 #include "../../include/grav.h"
 #include "psi.cuh"
-#include "psi2.cuh"
 
 namespace grav {
 
@@ -29,10 +28,12 @@ struct Geom {
 // Launch plans fixed at context creation (deterministic reduction orders).
 struct Plan {
     // forward: grid (obs tiles, node-column chunks)
-    int log2d;             // 1: kernels use the 2-D log table (psi2.cuh LOG2D)
-    int fwd_tpb, fwd_obs_per_thread, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
+    int log2d;             // 1: kernels use the 2-D log table (psi.cuh LOG2D)
+    int fwd_tpb, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
     // adjoint: grid (node-thread blocks, station chunks)
     int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;
+    // per-pair family (stored.cu): node tile of pair_tnx x pair_tny node columns per block
+    int pair_tnx, pair_tny, pair_tiles_x, pair_tiles_y, pair_zb_shift;
 };
 
 constexpr int kDotBlocks = 256;     // block partials of the fused CG dot products
@@ -42,14 +43,24 @@ constexpr int kDotThreads = 256;
 // scalar another block of the same launch writes.
 struct CgScalars {
     double rho[2];
-    double delta, a, b, dnorm2, tol2;
-    int done, iters_done;
+    double delta, a, b, dnorm2, tol2, rr;     // rr = ||r||^2 of the last finished iteration
+    int done, iters_done, it;                 // it: iteration counter of the current call (cg_advance_kernel)
 };
 
 struct WsLayout {
-    size_t cnode, tnode, fwd_partial, adj_partial, gcell, cg_x, cg_r, cg_p, cg_q, cg_w, dot_partial, scalars,
-        stage_m, stage_n, stage_hist, inv_dm, inv_r, inv_dd, inv_try, inv_scal, matfree_end, gemvt_partial, gstore;
+    size_t cnode, tnode, fwd_partial, adj_partial, gcell, cg_x, cg_r, cg_p, cg_q, cg_z, cg_w, dot_partial, scalars,
+        stage_m, stage_n, stage_hist, inv_dm, inv_r, inv_dd, inv_try, inv_scal, gram_partial, comm_gather, matfree_end,
+        gemvt_partial, gstore;
 };
+
+// (hi_out, lo_out) = (hi_in, lo_in) + x with the rounding error of hi_in + x captured exactly (Knuth TwoSum).
+__device__ __forceinline__ void two_sum_acc(double hi_in, double lo_in, double x, double& hi_out, double& lo_out) {
+    const double s = hi_in + x;
+    const double bb = s - hi_in;
+    const double err = (hi_in - (s - bb)) + (x - bb);
+    hi_out = s;
+    lo_out = lo_in + err;
+}
 
 }  // namespace grav
 
@@ -58,20 +69,23 @@ struct grav_ctx {
     grav::Plan plan;
     grav::WsLayout lay;
     int device;
-    void* geom_dev;          // one allocation holding xn,yn,zn,xo,yo,zo
+    void* geom_dev;          // one allocation holding xn,yn,zn,xo,yo,zo and the Psi tables
     char* ws;                // caller's workspace
     size_t ws_bytes;
     int stored_elem;         // 0 none, 8 FP64, 4 FP32
-    grav::PsiDev pd;         // Psi tables (inside geom_dev) and the global exponent offset k0
-    grav::Psi2Dev pd2;       // tables and constants of the second-generation evaluator (psi2.cuh), same k0
+    grav::PsiDev pd;         // Psi tables (inside geom_dev), constants and the global exponent offset k0
     int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
-    int tune[4];             // launch-variant selectors (grav_debug_set_tuning): 0 forward, 1 adjoint
-    grav_allreduce_fn allreduce;   // observation-sharded operation: sum over ranks (NULL = single rank)
-    void* allreduce_user;
+    int log2d_force;         // -1: the plan's choice; 0 / 1: force the 256-entry / the 2-D log table (diagnostic)
+    grav_comm comm;          // observation-sharded operation (world == 1: single rank, no callbacks)
     long long launches;
 };
 
 namespace grav {
+
+inline bool use_log2d(const grav_ctx* c) {
+    if (!c->pd.tab2d) return false;
+    return c->log2d_force < 0 ? c->plan.log2d != 0 : c->log2d_force != 0;
+}
 
 // Opt a kernel into > 48 KB of dynamic shared memory once per (kernel, device); thread-safe (the attribute is per
 // device, and setting it twice is harmless).
@@ -97,35 +111,34 @@ cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double sca
                                   double* d, double* dot_partial, const CgScalars* sc, cudaStream_t s);
 // --- adjoint.cu : tnode[n] = sum_i v_i Psi(node_n - obs_i)
 cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s);
-cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, double* tnode, cudaStream_t s);
+cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, int nchunk, double* tnode, cudaStream_t s);
 // --- cg.cu
-cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, double* x, double* r, double* p, double* dotp, int resume,
-                           cudaStream_t s);
+cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, const double* minv, double lam, double* x, double* r,
+                           double* z, double* p, double* dotp, int resume, cudaStream_t s);
 cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc, double rtol, int resume,
                                   const double* rho_in, double* hist, cudaStream_t s);
-cudaError_t launch_dot_pq(grav_ctx* c, const double* p, const double* q, double lam, double* q_out, double* dotp,
-                          const CgScalars* sc, cudaStream_t s);
+cudaError_t launch_dot_pq(grav_ctx* c, const double* p, double lam, double* q, double* dotp, const CgScalars* sc,
+                          cudaStream_t s);
 cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,
-                                const double* dotp_in, double* dotp_out, CgScalars* sc, int it, cudaStream_t s);
-cudaError_t launch_cg_update_p(grav_ctx* c, const double* r, double* p, const double* dotp, CgScalars* sc, int it,
-                               double rtol, double* hist_slot, double* ab_slot, cudaStream_t s);
+                                const double* minv, double lam, double* z, const double* dotp_in, double* dotp_out,
+                                CgScalars* sc, cudaStream_t s);
+cudaError_t launch_cg_update_p(grav_ctx* c, const double* z, double* p, const double* dotp, CgScalars* sc, double* hist,
+                               double* ab, cudaStream_t s);
 // --- stored.cu
 cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s);
 cudaError_t launch_gemv(grav_ctx* c, const void* G, int elem, const double* u, double* d, cudaStream_t s);
 cudaError_t launch_gemvt(grav_ctx* c, const void* G, int elem, const double* v, const double* w_or_null, double* g,
                          double* partial, cudaStream_t s);
-cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s);
+cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* partial, double* diag, cudaStream_t s);
 cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double lam, double* A, cudaStream_t s);
 cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
-cudaError_t launch_scale_cells(grav_ctx* c, double* g, const double* w, cudaStream_t s);
 int gemvt_chunks(long long N);
+void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p);
+size_t gram_partial_doubles(const Geom& g, const Plan& p);
 // --- invert.cu : vector kernels of the outer model-update loop
 cudaError_t launch_inv_residual(grav_ctx* c, const double* r, double s, const double* dd, double* out, double* partial,
                                 cudaStream_t st);
 cudaError_t launch_inv_finish(grav_ctx* c, const double* partial, double* scalar, cudaStream_t st);
-cudaError_t launch_inv_axpy(grav_ctx* c, double a, const double* x, const double* y0, double* y, cudaStream_t st);
-cudaError_t init_forward_kernels();
-cudaError_t init_adjoint_kernels();
-cudaError_t init_stored_kernels();
+cudaError_t launch_inv_axpy(grav_ctx* c, double a, const double* x, double* y, cudaStream_t st);
 
 }  // namespace grav

@@ -48,11 +48,10 @@ __global__ void __launch_bounds__(kDotBlocks) inv_finish_kernel(const double* __
     if (threadIdx.x == 0) *scalar = sh[0];
 }
 
-// y = (x0 ? x0 : 0) + a * x   (elementwise, M-vectors)
-__global__ void inv_axpy_kernel(long long M, double a, const double* __restrict__ x, const double* __restrict__ y0,
-                                double* __restrict__ y) {
+// y += a * x   (elementwise, M-vectors, in place)
+__global__ void inv_axpy_kernel(long long M, double a, const double* __restrict__ x, double* __restrict__ y) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < M) y[i] = fma(a, x[i], y0 ? y0[i] : 0.0);
+    if (i < M) y[i] = fma(a, x[i], y[i]);
 }
 
 cudaError_t launch_inv_residual(grav_ctx* c, const double* r, double s, const double* dd, double* out, double* partial,
@@ -66,8 +65,8 @@ cudaError_t launch_inv_finish(grav_ctx* c, const double* partial, double* scalar
     c->launches++;
     return cudaGetLastError();
 }
-cudaError_t launch_inv_axpy(grav_ctx* c, double a, const double* x, const double* y0, double* y, cudaStream_t st) {
-    inv_axpy_kernel<<<(unsigned)((c->g.M + 255) / 256), 256, 0, st>>>(c->g.M, a, x, y0, y);
+cudaError_t launch_inv_axpy(grav_ctx* c, double a, const double* x, double* y, cudaStream_t st) {
+    inv_axpy_kernel<<<(unsigned)((c->g.M + 255) / 256), 256, 0, st>>>(c->g.M, a, x, y);
     c->launches++;
     return cudaGetLastError();
 }

@@ -73,13 +73,6 @@ __global__ void node_to_cell_kernel(Geom g, const double* __restrict__ tnode, co
     gcell[cell] = val;
 }
 
-__global__ void scale_cells_kernel(long long M, double* __restrict__ g, const double* __restrict__ w) {
-    long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= M) return;
-    double ww = w[cell];
-    g[cell] = g[cell] / (ww * ww);
-}
-
 // w_k = (zc_k + z0)^(-beta/2)   (BASELINE.json north_star).  Depends on the layer only.
 __global__ void depth_weights_kernel(Geom g, double beta, double z0, double* __restrict__ w) {
     long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -99,11 +92,6 @@ cudaError_t launch_cell_to_node(grav_ctx* c, const double* u, const double* w, d
 cudaError_t launch_node_to_cell(grav_ctx* c, const double* tnode, const double* w, double scale, double* gcell,
                                 cudaStream_t s) {
     node_to_cell_kernel<<<blocks_for(c->g.M, 256), 256, 0, s>>>(c->g, tnode, w, scale, gcell);
-    c->launches++;
-    return cudaGetLastError();
-}
-cudaError_t launch_scale_cells(grav_ctx* c, double* g, const double* w, cudaStream_t s) {
-    scale_cells_kernel<<<blocks_for(c->g.M, 256), 256, 0, s>>>(c->g.M, g, w);
     c->launches++;
     return cudaGetLastError();
 }

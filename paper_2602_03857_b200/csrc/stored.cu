@@ -1,221 +1,189 @@
 // stored.cu -- the per-pair kernel family and the stored-G path (BASELINE.json north_star kernel 4).
 //
 // tabulate:  G[i][m] = gamma * sum_pqr sigma Psi(corner_pqr(m) - obs_i)   (Eq. 1; the paper's
-//            Listing 1, one thread per entry).  Here one thread evaluates the 4 corners of one
-//            horizontal node layer of a prism column, L(c) = sum_{da,db} (-1)^(da+db) Psi(X_da, Y_db, Z_c), and
-//            the prism between layers c and c+1 is gamma*(L(c+1) - L(c)) with L(c+1) taken from the next lane
-//            (warp shuffle): 4 evaluations per pair instead of 8, stores coalesced along the prism index.
+//            Listing 1, one thread per entry; "global memory (sensitivity matrix)").
+//            Node-shared here: every Psi(node - station) is a corner of up to 8 prisms, so a block takes one station
+//            and a tile of (tnx-1) x (tny-1) cell columns, its threads evaluate Psi down the tnx x tny NODE columns
+//            of the tile once - (1 + 1/t)^2 (nz+1)/nz ~ 1.15 evaluations per pair instead of 8 - and park the vertical
+//            differences Psi(k+1) - Psi(k) in shared memory; the entry of prism (i, j, k) is then the signed sum of
+//            the four differences at its corner columns, written with lanes along k (contiguous in G).
+// gram_diag: diag_i = sum_k G_ik^2 / w_k^2 with the same walk, nothing stored (reading C7; its sum is the trace
+//            that fixes lambda, and diag + lambda is the Jacobi preconditioner of the data-space CG).
 // gemv / gemvt: d = G u (row dots), g = G^T v (column sums), one streaming read of G each, FP64 accumulation
 //            ("matrix multiplications"); HBM-bound.
-// gram_diag: diag_i = sum_k G_ik^2 / w_k^2 with the same per-pair evaluation, nothing stored (reading C7).
 // form_A / cholesky: explicit N x N data-space system for tiny N (BASELINE.json config 1).
 #include "grav_internal.cuh"
 #include "psi.cuh"
-#include "psi2.cuh"
 
 namespace grav {
 
-// ---- per-pair evaluation ---------------------------------------------------------------------------------
-// Flattened "layer" index q = cc*nzp + c over cell columns cc = i*ny + j and node layers c = 0..nz.
-// A warp owns 32 consecutive q starting at 31*warp; lane l < 31 outputs the prism (cc, k=c) if c < nz.
-template <bool FAST>
-__device__ __forceinline__ double layer_value(const Geom& g, const Psi2TabView& tb, long long q, long long nq, double xo,
-                                              double yo, double zo, int& cc, int& c) {
-    q = q < nq ? q : nq - 1;
-    cc = (int)(q / g.nzp);
-    c = (int)(q - (long long)cc * g.nzp);
-    const int i = cc / g.ny, j = cc - i * g.ny;
-    const double X1 = g.xn[i] - xo, X2 = g.xn[i + 1] - xo;
-    const double Y1 = g.yn[j] - yo, Y2 = g.yn[j + 1] - yo;
-    const double Z = g.zn[c] - zo;
-    // (-1)^(da+db): (0,0)+, (1,0)-, (0,1)-, (1,1)+
-    double v;
-    if (FAST) {
-        const PsiColumn c11 = psi_column(X1, Y1), c21 = psi_column(X2, Y1), c12 = psi_column(X1, Y2),
-                        c22 = psi_column(X2, Y2);
-        v = c11.s * psi2_fast(tb, c11, Z);
-        v = fma(-c21.s, psi2_fast(tb, c21, Z), v);
-        v = fma(-c12.s, psi2_fast(tb, c12, Z), v);
-        v = fma(c22.s, psi2_fast(tb, c22, Z), v);
-    } else {
-        v = psi_libm(X1, Y1, Z, X1 * Y1, fma(Y1, Y1, X1 * X1));
-        v -= psi_libm(X2, Y1, Z, X2 * Y1, fma(Y1, Y1, X2 * X2));
-        v -= psi_libm(X1, Y2, Z, X1 * Y2, fma(Y2, Y2, X1 * X1));
-        v += psi_libm(X2, Y2, Z, X2 * Y2, fma(Y2, Y2, X2 * X2));
-    }
-    return v;
-}
+// ---- per-pair evaluation, node-shared --------------------------------------------------------------------
+constexpr int kPairTPB = 320;            // >= 17 x 17 node columns: 16 x 16 cell columns per tile
+constexpr int kPairU = 8;                // evaluations in flight per thread
+enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 
-template <typename T, int TPB, bool FAST>
-__global__ void __launch_bounds__(TPB) tabulate_kernel(Geom g, Psi2Dev pd, T* __restrict__ G) {
+// Work item = (station, tile), tile index fastest; blocks stride over the items.  Phase A: thread t < nnx * nny owns
+// node column (i0 + t / nny, j0 + t % nny): hoists once per item, then Psi down the column in batches of zb layers,
+// storing dPsi(k) = Psi(k+1) - Psi(k) at s_d[t * (zb + 1) + k - k0] (odd stride: conflict-free).  Phase B: entry
+// (li, lj, k) = gamma * ((d11 - d21) - d12 + d22) with lanes along k - the same pairing as node_to_cell (vertical
+// neighbours first: their Psi values are closest), so stored and matrix-free products agree to rounding.
+// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = with the 2-D log table.
+template <int MODE, int EV>
+__global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev pd, int tnx, int tny, int tiles_y,
+                                                               int ntiles, int zb_shift, void* __restrict__ Gout,
+                                                               const double* __restrict__ w,
+                                                               double* __restrict__ gram_partial) {
     extern __shared__ double2 s_tab[];
-    Psi2TabView tb;
-    if (FAST) tb = psi2_tables_to_smem(s_tab, pd);
-    const long long nq = (long long)g.nx * g.ny * g.nzp;
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * TPB + threadIdx.x) >> 5;
-    const long long q = warp * 31 + lane;
-    if (warp * 31 >= nq) return;
-    for (long long i = blockIdx.y; i < g.N; i += gridDim.y) {
-        int cc, c;
-        const double L = layer_value<FAST>(g, tb, q, nq, g.xo[i], g.yo[i], g.zo[i], cc, c);
-        const double Lnext = __shfl_down_sync(0xffffffffu, L, 1);
-        if (lane < 31 && q < nq && c < g.nz) {
-            const long long m = (long long)cc * g.nz + c;
-            G[i * g.M + m] = (T)(g.gamma * (Lnext - L));
-        }
-    }
-}
-
-
-// Column-walking tabulation (the default): one thread owns one cell column (i, j) and walks down its nz + 1 node
-// layers for one station after another.  Everything that depends only on (station, corner column) - the four
-// PsiColumn hoists - is computed once per column instead of once per layer, the four corner evaluations of a layer
-// are independent (4 evaluations in flight per thread), and the entry of prism k is gamma (L(k+1) - L(k)) with both
-// layer values formed by the same thread: 4 evaluations per pair, no shuffles, no 64-bit index divisions.
-// Lanes are neighbouring cell columns, so a warp's stores of one layer are nz elements apart; consecutive layers
-// fill the same 32-byte sectors, which L2 merges before they reach DRAM.
-template <typename T, int TPB, int EV>   // EV 2: 256-entry log table, 3: exponent-and-mantissa log table
-__global__ void __launch_bounds__(TPB) tabulate_cols_kernel(Geom g, Psi2Dev pd, T* __restrict__ G) {
-    extern __shared__ double2 s_tab[];
-    const Psi2TabView tb = EV == 3 ? psi2_tables_to_smem_2d(s_tab, pd) : psi2_tables_to_smem(s_tab, pd);
-    const int ncc = g.nx * g.ny;
-    const int cc = blockIdx.x * TPB + threadIdx.x;
-    const int ccl = cc < ncc ? cc : ncc - 1;
-    const int i = ccl / g.ny, j = ccl - i * g.ny;
-    const double x1 = g.xn[i], x2 = g.xn[i + 1], y1 = g.yn[j], y2 = g.yn[j + 1];
-    for (long long st = blockIdx.y; st < g.N; st += gridDim.y) {
+    __shared__ double s_red[kPairTPB / 32];
+    PsiTabView tb;
+    size_t tab_entries = 0;
+    if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); tab_entries = (size_t)kTabEntries * kRep; }
+    if (EV == 2) { tb = psi_tables_to_smem_2d(s_tab, pd); tab_entries = psi_log2d_smem_entries(pd); }
+    double* s_zn = reinterpret_cast<double*>(s_tab + tab_entries);
+    double* s_d = s_zn + ((g.nzp + 1) & ~1);
+    for (int c = threadIdx.x; c < g.nzp; c += kPairTPB) s_zn[c] = g.zn[c];
+    __syncthreads();
+    const int zb = 1 << zb_shift, stride = zb + 1;
+    const int t = threadIdx.x;
+    const long long nitems = g.N * (long long)ntiles;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const long long st = item / ntiles;
+        const int tile = (int)(item - st * ntiles);
+        const int tx = tile / tiles_y, ty = tile - tx * tiles_y;
+        const int i0 = tx * (tnx - 1), j0 = ty * (tny - 1);
+        const int nnx = min(tnx, g.nxp - i0), nny = min(tny, g.nyp - j0);       // node columns of this tile
+        const int ncx = nnx - 1, ncy = nny - 1;                                 // cell columns of this tile
+        const bool active = t < nnx * nny;
+        const int la = active ? t / nny : 0, lb = active ? t - la * nny : 0;
         const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
-        const PsiColumn c11 = psi_column(x1 - xo, y1 - yo), c21 = psi_column(x2 - xo, y1 - yo),
-                        c12 = psi_column(x1 - xo, y2 - yo), c22 = psi_column(x2 - xo, y2 - yo);
-        T* __restrict__ out = G + st * g.M + (long long)ccl * g.nz;
-        double Lprev = 0.0;
-#pragma unroll 2
-        for (int c = 0; c < g.nzp; ++c) {
-            const double Z = __ldg(g.zn + c) - zo;
-            // (-1)^(da+db): (0,0)+, (1,0)-, (0,1)-, (1,1)+   (same order as layer_value)
-            double L = c11.s * psi2_fast_t<EV == 3>(tb, c11, Z);
-            L = fma(-c21.s, psi2_fast_t<EV == 3>(tb, c21, Z), L);
-            L = fma(-c12.s, psi2_fast_t<EV == 3>(tb, c12, Z), L);
-            L = fma(c22.s, psi2_fast_t<EV == 3>(tb, c22, Z), L);
-            if (c > 0 && cc < ncc) out[c - 1] = (T)(g.gamma * (L - Lprev));
-            Lprev = L;
-        }
-    }
-}
-
-template <typename T, int EV>
-static cudaError_t tabulate_cols_launch(grav_ctx* c, T* G, cudaStream_t s) {
-    constexpr int TPB = 512;
-    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 : kTab2SmemBytes;
-    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
-    static unsigned long long smem_set = 0;
-    cudaError_t e = ensure_dynamic_smem(tabulate_cols_kernel<T, TPB, EV>, smem_max, c->device, &smem_set);
-    if (e != cudaSuccess) return e;
-    const int ncc = c->g.nx * c->g.ny;
-    const unsigned gx = (unsigned)((ncc + TPB - 1) / TPB);
-    // every block fills the tables once and then loops over its stations: ~16 blocks per SM in total
-    long long gy = (148LL * 16 + gx - 1) / gx;
-    if (gy > c->g.N) gy = c->g.N;
-    if (gy > 65535) gy = 65535;
-    if (gy < 1) gy = 1;
-    tabulate_cols_kernel<T, TPB, EV><<<dim3(gx, (unsigned)gy), TPB, smem, s>>>(c->g, c->pd2, G);
-    return cudaGetLastError();
-}
-
-template <int TPB, bool FAST>
-__global__ void __launch_bounds__(TPB) gram_diag_kernel(Geom g, Psi2Dev pd, const double* __restrict__ w,
-                                                         double* __restrict__ diag) {
-    extern __shared__ double2 s_tab[];
-    __shared__ double sh[TPB];
-    Psi2TabView tb;
-    if (FAST) tb = psi2_tables_to_smem(s_tab, pd);
-    const long long nq = (long long)g.nx * g.ny * g.nzp;
-    const int lane = threadIdx.x & 31;
-    const int warp_in_block = threadIdx.x >> 5;
-    constexpr int WPB = TPB / 32;
-    const long long nwarp_tasks = (nq + 30) / 31;
-    for (long long i = blockIdx.x; i < g.N; i += gridDim.x) {
-        const double xo = g.xo[i], yo = g.yo[i], zo = g.zo[i];
-        double acc = 0.0;
-        for (long long wt = warp_in_block; wt < nwarp_tasks; wt += WPB) {
-            const long long q = wt * 31 + lane;
-            int cc, c;
-            const double L = layer_value<FAST>(g, tb, q, nq, xo, yo, zo, cc, c);
-            const double Lnext = __shfl_down_sync(0xffffffffu, L, 1);
-            if (lane < 31 && q < nq && c < g.nz) {
-                const double gv = g.gamma * (Lnext - L);
-                const double ww = w[(long long)cc * g.nz + c];
-                acc = fma(gv / ww, gv / ww, acc);
-            }
-        }
-        sh[threadIdx.x] = acc;
-        __syncthreads();
-        for (int s = TPB / 2; s > 0; s >>= 1) {
-            if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
-            __syncthreads();
-        }
-        if (threadIdx.x == 0) diag[i] = sh[0];
-        __syncthreads();
-    }
-}
-
-
-// Gram diagonal with the same column walk: one block per station (grid-stride), its threads stride over the cell
-// columns, every thread accumulates G_ik^2 / w_k^2 down its columns; fixed-order block reduction.
-template <int TPB, int EV>
-__global__ void __launch_bounds__(TPB) gram_cols_kernel(Geom g, Psi2Dev pd, const double* __restrict__ w,
-                                                         double* __restrict__ diag) {
-    extern __shared__ double2 s_tab[];
-    __shared__ double sh[TPB];
-    const Psi2TabView tb = EV == 3 ? psi2_tables_to_smem_2d(s_tab, pd) : psi2_tables_to_smem(s_tab, pd);
-    const int ncc = g.nx * g.ny;
-    for (long long st = blockIdx.x; st < g.N; st += gridDim.x) {
-        const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
-        double acc = 0.0;
-        for (int cc = threadIdx.x; cc < ncc; cc += TPB) {
-            const int i = cc / g.ny, j = cc - i * g.ny;
-            const double x1 = g.xn[i] - xo, x2 = g.xn[i + 1] - xo, y1 = g.yn[j] - yo, y2 = g.yn[j + 1] - yo;
-            const PsiColumn c11 = psi_column(x1, y1), c21 = psi_column(x2, y1), c12 = psi_column(x1, y2),
-                            c22 = psi_column(x2, y2);
-            const double* __restrict__ wc = w + (long long)cc * g.nz;
-            double Lprev = 0.0;
-#pragma unroll 2
-            for (int c = 0; c < g.nzp; ++c) {
-                const double Z = __ldg(g.zn + c) - zo;
-                double L = c11.s * psi2_fast_t<EV == 3>(tb, c11, Z);
-                L = fma(-c21.s, psi2_fast_t<EV == 3>(tb, c21, Z), L);
-                L = fma(-c12.s, psi2_fast_t<EV == 3>(tb, c12, Z), L);
-                L = fma(c22.s, psi2_fast_t<EV == 3>(tb, c22, Z), L);
-                if (c > 0) {
-                    const double gv = g.gamma * (L - Lprev) / wc[c - 1];
-                    acc = fma(gv, gv, acc);
+        const double X = g.xn[i0 + la] - xo, Y = g.yn[j0 + lb] - yo;
+        PsiColumn pc;
+        double XY = 0.0, Q = 0.0;
+        if (EV != 0) pc = psi_column(X, Y);
+        else { XY = X * Y; Q = fma(Y, Y, X * X); }
+        auto eval = [&](int c) -> double {
+            const double Z = s_zn[c] - zo;
+            if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
+            return pc.s * psi_eval<EV == 2>(tb, pc, Z);
+        };
+        double prev = active ? eval(0) : 0.0;
+        double gram = 0.0;
+        for (int k0 = 0; k0 < g.nz; k0 += zb) {
+            const int nb = min(zb, g.nz - k0);
+            if (active) {
+                double* dst = s_d + t * stride;
+                // kPairU independent evaluations in flight; layers past the mesh bottom (last partial group only) are
+                // evaluated at the bottom layer and dropped
+                for (int kk = 0; kk < nb; kk += kPairU) {
+                    double cur[kPairU];
+#pragma unroll
+                    for (int u = 0; u < kPairU; ++u) cur[u] = eval(min(k0 + kk + u + 1, g.nz));
+                    double last = prev;
+#pragma unroll
+                    for (int u = 0; u < kPairU; ++u) {
+                        if (kk + u < nb) { dst[kk + u] = cur[u] - last; prev = cur[u]; }
+                        last = cur[u];
+                    }
                 }
-                Lprev = L;
             }
-        }
-        sh[threadIdx.x] = acc;
-        __syncthreads();
-        for (int k = TPB / 2; k > 0; k >>= 1) {
-            if (threadIdx.x < k) sh[threadIdx.x] += sh[threadIdx.x + k];
+            __syncthreads();
+            // phase B: flattened (cell column, layer) pairs, layer fastest
+            const int nent = (ncx * ncy) << zb_shift;
+            for (int e = t; e < nent; e += kPairTPB) {
+                const int cc = e >> zb_shift, l = e & (zb - 1);
+                if (l >= nb) continue;
+                const int li = cc / ncy, lj = cc - li * ncy;
+                const double* d11 = s_d + (li * nny + lj) * stride + l;
+                const double* d21 = d11 + nny * stride;
+                const double val = g.gamma * (((d11[0] - d21[0]) - d11[stride]) + d21[stride]);
+                const long long cell = ((long long)(i0 + li) * g.ny + (j0 + lj)) * g.nz + k0 + l;
+                if (MODE == PAIR_F64) reinterpret_cast<double*>(Gout)[st * g.M + cell] = val;
+                else if (MODE == PAIR_F32) reinterpret_cast<float*>(Gout)[st * g.M + cell] = (float)val;
+                else {
+                    const double q = val / w[cell];
+                    gram = fma(q, q, gram);
+                }
+            }
             __syncthreads();
         }
-        if (threadIdx.x == 0) diag[st] = sh[0];
-        __syncthreads();
+        if (MODE == PAIR_GRAM) {      // fixed-order block sum -> gram_partial[station][tile]
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) gram += __shfl_down_sync(0xffffffffu, gram, o);
+            if ((t & 31) == 0) s_red[t >> 5] = gram;
+            __syncthreads();
+            if (t == 0) {
+                double sum = 0.0;
+#pragma unroll
+                for (int k = 0; k < kPairTPB / 32; ++k) sum += s_red[k];
+                gram_partial[item] = sum;
+            }
+            __syncthreads();
+        }
     }
 }
 
-template <int EV>
-static cudaError_t gram_cols_launch(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
-    constexpr int TPB = 512;
-    constexpr size_t smem_max = EV == 3 ? kAtan2SmemBytes + (size_t)kLog2dMaxBinades * 4096 : kTab2SmemBytes;
-    const size_t smem = EV == 3 ? kAtan2SmemBytes + (size_t)c->pd2.nb2d * 4096 : smem_max;
+// diag[st] = sum over tiles of gram_partial[st][tile], in tile order
+__global__ void gram_reduce_kernel(long long N, int ntiles, const double* __restrict__ partial,
+                                   double* __restrict__ diag) {
+    const long long st = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (st >= N) return;
+    double s = 0.0;
+    for (int k = 0; k < ntiles; ++k) s += partial[st * ntiles + k];
+    diag[st] = s;
+}
+
+static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev, int zb_shift) {
+    const size_t tab = ev == 0 ? 0 : (ev == 2 ? psi_smem_bytes<true>(pd) : kTabSmemBytes);
+    return tab + (size_t)((g.nzp + 1) & ~1) * 8 + (size_t)kPairTPB * ((1 << zb_shift) + 1) * 8;
+}
+constexpr size_t kPairSmemMax = 227 * 1024;
+
+// Tile shape: tnx * tny <= kPairTPB node columns minimising the number of tiles (every tile costs one block the same
+// time), ties towards the squarer tile; batch depth 32 layers, 16 or 8 when the tables leave less shared memory.
+void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
+    long long best = -1;
+    p.pair_tnx = p.pair_tny = 2;
+    for (int tnx = 2; tnx <= kPairTPB / 2; ++tnx) {
+        const int tny = kPairTPB / tnx;
+        if (tny < 2) break;
+        const int ex = tnx > g.nxp ? g.nxp : tnx, ey = tny > g.nyp ? g.nyp : tny;      // never larger than the mesh
+        const long long tiles = (long long)((g.nx + ex - 2) / (ex - 1)) * ((g.ny + ey - 2) / (ey - 1));
+        const long long score = tiles * 1024 + (ex > ey ? ex - ey : ey - ex);
+        if (best < 0 || score < best) { best = score; p.pair_tnx = ex; p.pair_tny = ey; }
+    }
+    p.pair_tiles_x = (g.nx + p.pair_tnx - 2) / (p.pair_tnx - 1);
+    p.pair_tiles_y = (g.ny + p.pair_tny - 2) / (p.pair_tny - 1);
+    p.pair_zb_shift = 5;
+    while (p.pair_zb_shift > 3 && pair_smem_bytes(g, pd, log2d ? 2 : 1, p.pair_zb_shift) > kPairSmemMax) --p.pair_zb_shift;
+}
+
+size_t gram_partial_doubles(const Geom& g, const Plan& p) { return (size_t)g.N * p.pair_tiles_x * p.pair_tiles_y; }
+
+template <int MODE, int EV>
+static cudaError_t pair_launch(grav_ctx* c, void* G, const double* w, double* gram_partial, cudaStream_t s) {
+    const Plan& p = c->plan;
+    const size_t smem = pair_smem_bytes(c->g, c->pd, EV, p.pair_zb_shift);
+    if (smem > kPairSmemMax) return cudaErrorInvalidValue;          // node columns deeper than ~20,000 layers
     static unsigned long long smem_set = 0;
-    cudaError_t e = ensure_dynamic_smem(gram_cols_kernel<TPB, EV>, smem_max, c->device, &smem_set);
+    cudaError_t e = ensure_dynamic_smem(pair_tile_kernel<MODE, EV>, kPairSmemMax, c->device, &smem_set);
     if (e != cudaSuccess) return e;
-    const unsigned blocks = (unsigned)(c->g.N < 148 * 16 ? c->g.N : 148 * 16);
-    gram_cols_kernel<TPB, EV><<<blocks, TPB, smem, s>>>(c->g, c->pd2, w, diag);
+    const int ntiles = p.pair_tiles_x * p.pair_tiles_y;
+    const long long nitems = c->g.N * (long long)ntiles;
+    int sms = 148;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) sms = 148;
+    const unsigned blocks = (unsigned)(nitems < sms ? nitems : sms);    // one resident block per SM (shared memory)
+    pair_tile_kernel<MODE, EV><<<blocks, kPairTPB, smem, s>>>(c->g, c->pd, p.pair_tnx, p.pair_tny, p.pair_tiles_y,
+                                                               ntiles, p.pair_zb_shift, G, w, gram_partial);
     return cudaGetLastError();
+}
+
+template <int MODE>
+static cudaError_t pair_dispatch(grav_ctx* c, void* G, const double* w, double* gram_partial, cudaStream_t s) {
+    if (c->psi_variant == 1) return pair_launch<MODE, 0>(c, G, w, gram_partial, s);
+    // the 2-D log table only when it leaves room for the tile buffer
+    if (use_log2d(c) && pair_smem_bytes(c->g, c->pd, 2, c->plan.pair_zb_shift) <= kPairSmemMax)
+        return pair_launch<MODE, 2>(c, G, w, gram_partial, s);
+    return pair_launch<MODE, 1>(c, G, w, gram_partial, s);
 }
 
 // ---- GEMV: d = G u ----------------------------------------------------------------------------------------
@@ -383,49 +351,19 @@ __global__ void __launch_bounds__(1024) cholesky_solve_kernel(double* __restrict
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------
-static unsigned pair_blocks(const Geom& g, int tpb) {
-    const long long nq = (long long)g.nx * g.ny * g.nzp;
-    const long long nwarps = (nq + 30) / 31;
-    return (unsigned)((nwarps * 32 + tpb - 1) / tpb);
-}
-
-cudaError_t init_stored_kernels() {
-    cudaError_t e = cudaFuncSetAttribute(tabulate_kernel<double, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tabulate_kernel<float, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(gram_diag_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTab2SmemBytes);
+cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
+    cudaError_t e = elem == 8 ? pair_dispatch<PAIR_F64>(c, G, nullptr, nullptr, s)
+                              : pair_dispatch<PAIR_F32>(c, G, nullptr, nullptr, s);
+    c->launches++;
     return e;
 }
 
-cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
-    dim3 grid(pair_blocks(c->g, 256), (unsigned)(c->g.N < 65535 ? c->g.N : 65535));
-    if (c->psi_variant == 0 && c->tune[2] == 0) {          // default: column-walking kernel
-        cudaError_t e;
-        if (c->plan.log2d) e = elem == 8 ? tabulate_cols_launch<double, 3>(c, (double*)G, s) : tabulate_cols_launch<float, 3>(c, (float*)G, s);
-        else e = elem == 8 ? tabulate_cols_launch<double, 2>(c, (double*)G, s) : tabulate_cols_launch<float, 2>(c, (float*)G, s);
-        c->launches++;
-        return e;
-    }
-    if (c->psi_variant == 0) {                              // tune[2] = 1: layer-per-thread kernel (A/B)
-        if (elem == 8) tabulate_kernel<double, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (double*)G);
-        else tabulate_kernel<float, 256, true><<<grid, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, (float*)G);
-    } else {
-        if (elem == 8) tabulate_kernel<double, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd2, (double*)G);
-        else tabulate_kernel<float, 256, false><<<grid, 256, 0, s>>>(c->g, c->pd2, (float*)G);
-    }
-    c->launches++;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* diag, cudaStream_t s) {
-    unsigned blocks = (unsigned)(c->g.N < (1 << 20) ? c->g.N : (1 << 20));
-    if (c->psi_variant == 0 && c->tune[2] == 0) {          // default: column-walking kernel
-        cudaError_t e = c->plan.log2d ? gram_cols_launch<3>(c, w, diag, s) : gram_cols_launch<2>(c, w, diag, s);
-        c->launches++;
-        return e;
-    }
-    if (c->psi_variant == 0) gram_diag_kernel<256, true><<<blocks, 256, kTab2SmemBytes, s>>>(c->g, c->pd2, w, diag);
-    else gram_diag_kernel<256, false><<<blocks, 256, 0, s>>>(c->g, c->pd2, w, diag);
-    c->launches++;
+cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* partial, double* diag, cudaStream_t s) {
+    cudaError_t e = pair_dispatch<PAIR_GRAM>(c, nullptr, w, partial, s);
+    if (e != cudaSuccess) return e;
+    gram_reduce_kernel<<<(unsigned)((c->g.N + 255) / 256), 256, 0, s>>>(c->g.N, c->plan.pair_tiles_x * c->plan.pair_tiles_y,
+                                                                        partial, diag);
+    c->launches += 2;
     return cudaGetLastError();
 }
 

@@ -3,13 +3,15 @@
 The path shards the way the paper shards it ("observation domain partitioned across devices,
 model-space variables replicated and synchronised"): rank r owns a contiguous block of stations and the whole mesh.
   forward  d = G u      : rows of d are local -- no communication;
-  adjoint  g = G^T v    : every rank forms the node sums T over ITS stations, one all-reduce(sum) of T (2 N_n doubles: high and low
-                          parts of the compensated sums, 54 MB at config 5) makes them global -- the only data-path collective;
+  adjoint  g = G^T v    : every rank forms the node sums T over ITS stations as compensated (hi, lo) pairs; one
+                          all-gather of those planes (2 N_n doubles per rank, 54 MB at config 5) and an error-free
+                          combination in rank order (csrc/adjoint.cu adjoint_reduce) make them global and bit-identical
+                          on every rank -- the only data-path collective;
   CG                    : alpha, x, r, p, q are station vectors (local rows); each dot product all-reduces its 256
                           block partials, so every rank computes bit-identical scalars on the device.
-The exchanges are issued by libgrav.so itself through the hook of include/grav.h (grav_set_allreduce); this module
-only provides the hook (an NCCL all-reduce on a tensor view of the buffer) and the station partition.  Nothing here
-computes any part of the method.
+The exchanges are issued by libgrav.so itself through the callbacks of include/grav.h (grav_set_comm); this module
+only provides the callbacks (NCCL collectives on tensor views of the raw buffers) and the station partition.  Nothing
+here computes any part of the method.
 """
 import os
 
@@ -35,19 +37,20 @@ class _RawDeviceArray:
                                          "version": 2}
 
 
-class AllReduceHook:
-    """Callable for GravContext.set_allreduce: sums `count` doubles at a raw address, in place, over `group`.
+class Comm:
+    """Collectives for GravContext.set_comm on raw addresses, over `group`.
 
-    device = a CUDA device: the buffer is viewed zero-copy as a float64 tensor and reduced with NCCL; the collective
-    is ordered after the work already enqueued on the current stream and the current stream waits for it (torch's
-    synchronous all_reduce semantics), which is the stream libgrav.so was given.
-    device = "cpu": host address (gloo; used by the CPU tests of this plumbing)."""
+    device = a CUDA device: buffers are viewed zero-copy as float64 tensors and the NCCL collective is issued under
+    torch.cuda.stream(ExternalStream(stream)) - the stream libgrav.so hands over - so it is ordered with the library's
+    kernels whatever torch's current stream is.
+    device = "cpu": host addresses (gloo; used by the CPU tests of this plumbing)."""
 
     def __init__(self, device, group=None):
         self.device = torch.device(device)
         self.group = group
-        self.calls = 0
-        self.elements = 0
+        self.world = dist.get_world_size(group) if dist.is_initialized() else 1
+        self.rank = dist.get_rank(group) if dist.is_initialized() else 0
+        self.calls = []           # ("allreduce" | "allgather", count) in call order
 
     def view(self, ptr: int, count: int) -> torch.Tensor:
         if self.device.type == "cuda":
@@ -55,11 +58,24 @@ class AllReduceHook:
         import ctypes
         return torch.from_numpy(np.ctypeslib.as_array((ctypes.c_double * count).from_address(ptr)))
 
-    def __call__(self, ptr: int, count: int, stream: int = 0):
-        v = self.view(ptr, count)
-        dist.all_reduce(v, op=dist.ReduceOp.SUM, group=self.group)
-        self.calls += 1
-        self.elements += count
+    def _on(self, stream: int):
+        if self.device.type != "cuda":
+            import contextlib
+            return contextlib.nullcontext()
+        if stream == 0:           # the legacy default stream cannot be wrapped; torch's default stream is that stream
+            return torch.cuda.stream(torch.cuda.default_stream(self.device))
+        return torch.cuda.stream(torch.cuda.ExternalStream(stream, device=self.device))
+
+    def allreduce_sum(self, ptr: int, count: int, stream: int = 0):
+        with self._on(stream):
+            dist.all_reduce(self.view(ptr, count), op=dist.ReduceOp.SUM, group=self.group)
+        self.calls.append(("allreduce", count))
+
+    def allgather(self, send_ptr: int, recv_ptr: int, count: int, stream: int = 0):
+        with self._on(stream):
+            dist.all_gather_into_tensor(self.view(recv_ptr, count * self.world), self.view(send_ptr, count),
+                                        group=self.group)
+        self.calls.append(("allgather", count))
 
 
 def init_from_env(backend="nccl"):
@@ -88,10 +104,10 @@ class ShardedContext:
         sl = slice(self.lo, self.hi)
         self.ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo[sl], wl.yo[sl], wl.zo[sl], wl.gamma, device=local,
                                        mode=mode)
-        self.hook = None
+        self.comm = None
         if world > 1:
-            self.hook = AllReduceHook(self.ctx.device)
-            self.ctx.set_allreduce(self.hook)
+            self.comm = Comm(self.ctx.device)
+            self.ctx.set_comm(self.comm)
 
     def local(self, a):
         """Rows of a station vector (numpy) owned by this rank, as a device tensor."""

@@ -1,8 +1,8 @@
-"""Multi-rank host logic on CPU (gloo, world_size 2): the station partition, the all-reduce hook's raw-address view,
-and the placement of the exchanges -- an observation-sharded CG that all-reduces the adjoint
-output and the dot-product partials reproduces the unsharded CG.  The local operators in that check are the
-oracle's (tests may use it); the CUDA kernels cannot run here, their sharded use is covered on the GPU by
-tests/test_gpu_parity.py::test_allreduce_hook_placement.
+"""Multi-rank host logic on CPU (gloo, world_size 2): the station partition, the collectives of dist.Comm on raw
+addresses, and the placement of the exchanges -- an observation-sharded CG that sums the adjoint
+output and the dot-product partials over ranks reproduces the unsharded CG.  The local operators in that check are
+the oracle's (tests may use it); the CUDA kernels cannot run here, their sharded use is covered on the GPU by
+tests/test_gpu_parity.py::test_comm_exchange_placement and tests/test_gpu_multirank.py.
 """
 import os
 import socket
@@ -44,13 +44,19 @@ def _worker(rank, world, port, out):
     r, w, _ = gdist.init_from_env("gloo")
     assert (r, w) == (rank, world)
     try:
-        # ---- hook: raw host address -> in-place sum over ranks
-        hook = gdist.AllReduceHook("cpu")
+        # ---- collectives on raw host addresses: in-place sum over ranks, gather in rank order
+        comm = gdist.Comm("cpu")
+        assert (comm.world, comm.rank) == (world, rank)
         buf = np.arange(10, dtype=np.float64) * (rank + 1)
-        hook(buf.ctypes.data + 16, 5)                       # elements 2..6 only
+        comm.allreduce_sum(buf.ctypes.data + 16, 5)         # elements 2..6 only
         exp = np.arange(10, dtype=np.float64) * (rank + 1)
         exp[2:7] = np.arange(2, 7) * sum(range(1, world + 1))
-        assert np.array_equal(buf, exp) and hook.calls == 1 and hook.elements == 5
+        assert np.array_equal(buf, exp)
+        send = np.arange(4, dtype=np.float64) + 10 * rank
+        recv = np.full(4 * world + 1, -1.0)
+        comm.allgather(send.ctypes.data, recv.ctypes.data, 4)
+        assert np.array_equal(recv[:-1], np.concatenate([np.arange(4.0) + 10 * r for r in range(world)])) and recv[-1] == -1
+        assert comm.calls == [("allreduce", 5), ("allgather", 4)]
         assert gdist.max_over_ranks(float(rank + 1), "cpu") == float(world)
 
         # ---- exchange placement: sharded CG == unsharded CG (oracle operators, config 1)

@@ -1,5 +1,6 @@
 """CPU-only check of the hand-built Psi evaluator of csrc/psi.cuh (host emulation of the same source, MUFU seeds
-emulated at 2^-20) against the long-double oracle Psi: algorithm, tables and guards."""
+emulated at 2^-20) against the long-double oracle Psi: algorithm, tables and guards, with the 256-entry log table and
+with the exponent-and-mantissa ("2-D") log table."""
 import math
 
 import numpy as np
@@ -11,18 +12,18 @@ from paper_2602_03857_b200 import binding
 LN2 = math.log(2.0)
 
 
-GEN = 1      # evaluator generation under test (set by the autouse fixture: every test runs for psi.cuh and psi2.cuh)
+LOG2D = False      # log table under test (set by the autouse fixture: every test runs for both)
 
 
-@pytest.fixture(autouse=True, params=[1, 2, 3], ids=["psi", "psi2", "psi2-log2d"])
-def _generation(request):
-    global GEN
-    GEN = request.param
+@pytest.fixture(autouse=True, params=[False, True], ids=["log256", "log2d"])
+def _table(request):
+    global LOG2D
+    LOG2D = request.param
     yield
 
 
 def _scaled_err(X, Y, Z, k0=0):
-    got = binding.psi_fast_host(X, Y, Z, k0, GEN) - (X + Y) * k0 * LN2
+    got = binding.psi_eval_host(X, Y, Z, k0, LOG2D) - (X + Y) * k0 * LN2
     ref = oracle.psi(X, Y, Z, 1)
     R = math.sqrt(X * X + Y * Y + Z * Z)
     if R == 0:
@@ -48,10 +49,10 @@ def test_psi_fast_random(scale):
 def test_psi_fast_guards_and_special_points():
     pts = [(0, 0, 0), (0, -5, 0), (2, 3, 0), (0, 0, 5), (1, 1, 1), (3, -4, 0), (-3, 4, 1e-9), (0, 5, 2),
            (5, 0, 2), (-5, 0, -2), (1e-8, -1e4, 1e-8), (7, 7, 7), (7, -7, -7)]
-    if GEN == 3:      # the 2-D log table is only used when the geometry keeps R+Y, R+X inside its binades (never 0)
+    if LOG2D:         # the 2-D log table is only used when the geometry keeps R+Y, R+X inside its binades (never 0)
         pts = [a for a in pts if math.sqrt(sum(v * v for v in a)) + min(a[0], a[1]) > 1e-22]
     for args in pts:
-        got = binding.psi_fast_host(*args, 0, GEN)
+        got = binding.psi_eval_host(*args, 0, LOG2D)
         assert math.isfinite(got)
         ref = oracle.psi(*args, 1)
         assert abs(got - ref) <= 1e-15 * max(1.0, abs(ref)) + 1e-12 * (args == (1e-8, -1e4, 1e-8))

@@ -271,11 +271,13 @@ def test_libm_variant_matches(cfg1):
     ctx.close()
 
 
-@pytest.mark.parametrize("shape", [(9, 7, 12, 700), (3, 4, 70, 300), (2, 2, 1100, 40)])
+@pytest.mark.parametrize("shape", [(9, 7, 12, 700), (3, 4, 70, 300), (2, 2, 1100, 40), (6, 5, 8, 333), (4, 6, 11, 90),
+                                   (5, 3, 3, 64)])
 def test_launch_variants_against_oracle(shape):
-    """Every forward / adjoint launch variant (staged and unstaged z-stream, first- and second-generation Psi
-    evaluator, every KC) against the oracle on a ragged case spanning several station tiles, several staged
-    column tiles and a column deeper than the stage buffer (nz + 1 > 1024: unstaged fallback)."""
+    """Both log tables (256-entry and exponent-and-mantissa), the CUDA-libm evaluator and every compiled KC of the
+    adjoint kernel against the oracle, on ragged cases spanning several station tiles, several staged column tiles and
+    a column deeper than the stage buffer (nz + 1 > 1024: unstaged fallback).  nz + 1 = 13, 71, 9, 12, 4 make the plan
+    pick KC = 5, 8, 5, 6, 4 (csrc/grav_api.cu make_plan)."""
     nx, ny, nz, nobs = shape
     wl = workloads.make_custom(nx, ny, nz, 17.0, nobs, seed=5 + nz, topo_amp=25.0)
     mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
@@ -283,17 +285,22 @@ def test_launch_variants_against_oracle(shape):
     u, v = rng.standard_normal(wl.M), rng.standard_normal(wl.N)
     d_ref = oracle.forward(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, u)
     g_ref = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v)
-    ctx = make_ctx(wl)
-    # the 2-D log table exists for the first two shapes (variants 6-9 force it; it is the default only from 5e7
-    # evaluations per product); the 1100-layer mesh is 5e5 m deep under stations 1 m above it (4 Rmax^2 / Zmin^2 > 2^40)
+    G_ref = oracle.tabulate(mesh, wl.xo, wl.yo, wl.zo, wl.gamma) if wl.N * wl.M <= 4e6 else None
+    ctx = make_ctx(wl, mode=1 if G_ref is not None else 0)
+    # the 2-D log table exists for all but the 1100-layer mesh, which is 5e5 m deep under stations 1 m above it
+    # (4 Rmax^2 / Zmin^2 > 2^40); it is the default only from 5e7 evaluations per product
     assert (ctx.log2d_binades > 0) == (nz < 1000) and not ctx.log2d_default
-    for variant in range(11):
-        if ctx.log2d_binades == 0 and variant in (6, 7, 8, 9):
+    for log2d in (0, 1):
+        if log2d and ctx.log2d_binades == 0:
+            with pytest.raises(Exception):
+                ctx.set_log2d(1)
             continue
-        ctx.set_tuning(0, variant)
-        ctx.set_tuning(1, variant)
-        assert relmax(host(ctx.forward(dev(u))), d_ref) <= TOL_OP, f"forward variant {variant}"
-        assert relmax(host(ctx.adjoint(dev(v))), g_ref) <= TOL_OP, f"adjoint variant {variant}"
+        ctx.set_log2d(log2d)
+        assert relmax(host(ctx.forward(dev(u))), d_ref) <= TOL_OP, f"forward log2d={log2d}"
+        assert relmax(host(ctx.adjoint(dev(v))), g_ref) <= TOL_OP, f"adjoint log2d={log2d}"
+        if G_ref is not None:
+            ctx.store_g()
+            assert relmax(host(ctx.stored_g()), G_ref) <= TOL_OP, f"tabulate log2d={log2d}"
     ctx.close()
 
 
@@ -309,9 +316,8 @@ def test_survey_coordinates_with_large_offsets():
     u, v = rng.standard_normal(wl.M), rng.standard_normal(wl.N)
     ctx = binding.GravContext(xn, yn, zn, xo, yo, zo, wl.gamma, device=0)
     assert ctx.log2d_binades > 0
-    for variant in (0, 6):                                    # 256-entry table (small problem default) and 2-D table
-        ctx.set_tuning(0, variant)
-        ctx.set_tuning(1, variant)
+    for log2d in (0, 1):                                      # 256-entry table (small problem default) and 2-D table
+        ctx.set_log2d(log2d)
         assert relmax(host(ctx.forward(dev(u))), oracle.forward(mesh, xo, yo, zo, wl.gamma, u)) <= TOL_OP
         assert relmax(host(ctx.adjoint(dev(v))), oracle.adjoint(mesh, xo, yo, zo, wl.gamma, v)) <= TOL_OP
     ctx.close()
@@ -342,41 +348,53 @@ def test_log2d_admissibility():
     assert ctx.log2d_binades > 0
     ref = oracle.forward(mesh, base.xo, base.yo, zo, base.gamma, u)
     g_ref = oracle.adjoint(mesh, base.xo, base.yo, zo, base.gamma, ref)
-    for variant in (0, 6):
-        ctx.set_tuning(0, variant)
-        ctx.set_tuning(1, variant)
+    for log2d in (0, 1):
+        ctx.set_log2d(log2d)
         assert relmax(host(ctx.forward(dev(u))), ref) <= TOL_OP
         assert relmax(host(ctx.adjoint(dev(ref))), g_ref) <= TOL_OP
     ctx.close()
 
 
-def test_allreduce_hook_placement(cfg1):
-    """Observation sharding (include/grav.h: grav_set_allreduce).  Two IDENTICAL ranks, each holding the same
-    stations S, form the global system [G_S; G_S]; its all-reduce is "multiply by 2".  By symmetry the sharded CG must
-    then reproduce the single-rank CG of the problem with gamma*sqrt(2) (A = 2 G W^-2 G^T + lambda I): same alpha,
-    residual history and model larger by sqrt(2).  Every exchange point has to be hooked for this to hold."""
-    from paper_2602_03857_b200 import binding, dist as gdist
+class _TwinComm:
+    """Stand-in for a 2-rank communicator whose other rank holds the SAME stations: an all-reduce doubles the buffer,
+    an all-gather places two copies of the send buffer.  Runs on the stream it is handed."""
+
+    def __init__(self, device):
+        from paper_2602_03857_b200 import dist as gdist
+        self._c = gdist.Comm(device)
+        self.world, self.rank, self.calls = 2, 0, []
+
+    def allreduce_sum(self, ptr, count, stream):
+        with self._c._on(stream):
+            self._c.view(ptr, count).mul_(2.0)
+        self.calls.append(("allreduce", count))
+
+    def allgather(self, send, recv, count, stream):
+        with self._c._on(stream):
+            r = self._c.view(recv, 2 * count)
+            r[:count].copy_(self._c.view(send, count))
+            r[count:].copy_(self._c.view(send, count))
+        self.calls.append(("allgather", count))
+
+
+def test_comm_exchange_placement(cfg1):
+    """Observation sharding (include/grav.h: grav_set_comm).  Two IDENTICAL ranks, each holding the same stations S,
+    form the global system [G_S; G_S].  By symmetry the sharded CG must then reproduce the single-rank CG of the problem
+    with gamma*sqrt(2) (A = 2 G W^-2 G^T + lambda I): same alpha, residual history and model larger by sqrt(2).  Every
+    exchange point has to be hooked for this to hold."""
+    from paper_2602_03857_b200 import binding
     wl, w, lam, d = cfg1["wl"], cfg1["w"], cfg1["lam"], cfg1["d_obs"]
-    calls = []
-
-    def make_hook(ctx):
-        view = gdist.AllReduceHook(ctx.device).view
-
-        def hook(ptr, count, stream):
-            calls.append(count)
-            view(ptr, count).mul_(2.0)          # sum over two identical ranks, on the current stream
-        return hook
-
     its = 8
     for mode in (0, 1):
         sh = make_ctx(wl, mode=mode)
-        sh.set_allreduce(make_hook(sh))
+        comm = _TwinComm(sh.device)
+        sh.set_comm(comm)
         ref = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma * np.sqrt(2.0), device=0,
                                   mode=mode)
         if mode == 1:
             sh.store_g()
             ref.store_g()
-        calls.clear()
+        comm.calls.clear()
         a = sh.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
         b = ref.dataspace_cg(dev(d), dev(w), lam, its, mode=mode)
         # the two runs differ by rounding only (gamma*sqrt(2) is rounded), amplified over 8 CG iterations
@@ -384,17 +402,20 @@ def test_allreduce_hook_placement(cfg1):
         assert relmax(host(a["alpha"]), host(b["alpha"])) <= 1e-7
         assert np.abs(host(a["hist"]) / (np.sqrt(2.0) * host(b["hist"])) - 1).max() <= 1e-7
         assert relmax(host(a["m"]), np.sqrt(2.0) * host(b["m"])) <= 1e-7
-        big = 2 * wl.n_nodes if mode == 0 else wl.M     # node sums travel as (hi, lo) planes
-        # d.d, then per iteration: operator output, p.q, r.r; finally the model recovery
-        assert calls == [256] + [big, 256, 256] * its + [big]
+        # node sums travel as gathered (hi, lo) planes, the stored-mode M-vector as an all-reduce
+        big = ("allgather", 2 * wl.n_nodes) if mode == 0 else ("allreduce", wl.M)
+        # [r.z | d.d | r.r], then per iteration: operator output, p.q, [r.z | r.r]; finally the model recovery
+        assert comm.calls == [("allreduce", 768)] + [big, ("allreduce", 256), ("allreduce", 512)] * its + [big]
         # the adjoint is global (summed over the two ranks), the forward stays local
         v = cfg1["d_obs"]
-        calls.clear()
+        comm.calls.clear()
         g2 = host(sh.adjoint(dev(v)) if mode == 0 else sh.adjoint_stored(dev(v)))
-        assert calls == [big]
-        sh.set_allreduce(None)
+        assert comm.calls == [big]
+        sh.set_comm(None)
+        if mode == 1:
+            sh.store_g()
         g1 = host(sh.adjoint(dev(v)) if mode == 0 else sh.adjoint_stored(dev(v)))
-        assert np.array_equal(g2, 2.0 * g1) and len(calls) == 1
+        assert np.array_equal(g2, 2.0 * g1) and len(comm.calls) == 1
         with_hook_fwd = host(sh.forward(dev(wl.m_true)))
         assert relmax(with_hook_fwd, np.sqrt(0.5) * host(ref.forward(dev(wl.m_true)))) <= 1e-13
         sh.close()
