@@ -138,14 +138,16 @@ grav_status grav_direct_solve(grav_ctx* ctx, const double* dobs_dev, const doubl
  *   alpha = CG on (G W^-2 G^T + lambda I) alpha = r_k, <= max_inner iterations, stopped at ||res|| <= tol_inner ||r_k||;
  *   delta_m = W^-2 G^T alpha;  s = 1, halved at most 10 times until ||r_k - s G delta_m|| < ||r_k||
  *   (no decrease: stop with m_k);  m_{k+1} = m_k + s delta_m.
- * dobs_dev[N], w_dev[M], mref_dev[M] or NULL, m_dev[M] out, dpred_dev[N] out or NULL (= G m): DEVICE.
+ * dobs_dev[N], w_dev[M], mref_dev[M] or NULL, precond_dev[N] or NULL (Jacobi preconditioner of the inner solves, as in
+ * grav_dataspace_cg), m_dev[M] out, dpred_dev[N] out or NULL (= G m): DEVICE.
  * hist_host[max_outer + 1] (||r_k|| / ||d_obs||, entries 0..*n_outer_host), step_host[max_outer] (accepted s per
- * update, 0 = rejected), n_outer_host (updates applied): HOST, each may be NULL.  mode as in grav_dataspace_cg.
+ * update, 0 = rejected), inner_host[max_outer] (CG iterations each update performed before its tolerance stop),
+ * n_outer_host (updates applied): HOST, each may be NULL.  mode as in grav_dataspace_cg.
  * SYNCHRONISES the stream once per trial step (one scalar read back); needs the workspace. */
 grav_status grav_invert(grav_ctx* ctx, const double* dobs_dev, const double* w_dev, double lambda,
-                        const double* mref_dev, int max_outer, int max_inner, double tol_outer, double tol_inner,
-                        int mode, double* m_dev, double* dpred_dev, double* hist_host, double* step_host,
-                        int* n_outer_host, void* stream);
+                        const double* mref_dev, const double* precond_dev, int max_outer, int max_inner,
+                        double tol_outer, double tol_inner, int mode, double* m_dev, double* dpred_dev,
+                        double* hist_host, double* step_host, int* inner_host, int* n_outer_host, void* stream);
 
 /* End-to-end variants with HOST buffers: host->device copy of the inputs, the same kernels, device->host copy
  * of the result, then cudaStreamSynchronize(stream).  Staging buffers live in the workspace. */

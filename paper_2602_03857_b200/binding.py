@@ -95,7 +95,8 @@ def load():
     L.grav_fp64_peak_probe.restype = i
     L.grav_fp64_peak_probe.argtypes = [i, i, dp, dp]
     L.grav_invert.restype = i
-    L.grav_invert.argtypes = [vp, vp, vp, d, vp, i, i, d, d, i, vp, vp, vp, vp, C.POINTER(C.c_int), vp]
+    L.grav_invert.argtypes = [vp, vp, vp, d, vp, vp, i, i, d, d, i, vp, vp, vp, vp, C.POINTER(C.c_int),
+                              C.POINTER(C.c_int), vp]
     L.grav_debug_set_psi_variant.restype = i
     L.grav_debug_set_psi_variant.argtypes = [vp, i]
     L.grav_debug_psi_eval_host.restype = d
@@ -245,22 +246,25 @@ class GravContext:
         return dict(alpha=alpha, m=m, hist=hist, ab=ab[:2 * iters].view(-1, 2) if iters else ab[:0])
 
     def invert(self, dobs, w, lam, mref=None, max_outer=30, max_inner=20, tol_outer=1e-4, tol_inner=1e-4,
-               mode=MATRIX_FREE, want_dpred=True):
+               mode=MATRIX_FREE, want_dpred=True, precond=None):
         """The paper's outer model-update loop (include/grav.h: grav_invert).  Returns dict(m, dpred, hist, steps,
-        n_outer); hist / steps are numpy arrays."""
+        inner, n_outer, stop); hist / steps / inner (CG iterations per update) are numpy arrays."""
         m = self._new(self.M)
         dpred = self._new(self.N) if want_dpred else None
         hist = np.zeros(max_outer + 1)
         steps = np.zeros(max(max_outer, 1))
         n_outer = C.c_int(0)
+        inner = (C.c_int * max(max_outer, 1))()
         _check(self._lib.grav_invert(self._h, _dev(dobs, self.N, "dobs"), _dev(w, self.M, "w"), float(lam),
-                                     _dev(mref, self.M, "mref"), int(max_outer), int(max_inner), float(tol_outer),
-                                     float(tol_inner), int(mode), _dev(m, self.M, "m"), _dev(dpred, self.N, "dpred"),
-                                     C.c_void_p(hist.ctypes.data), C.c_void_p(steps.ctypes.data), C.byref(n_outer),
-                                     _stream()))
+                                     _dev(mref, self.M, "mref"), _dev(precond, self.N, "precond"), int(max_outer),
+                                     int(max_inner), float(tol_outer), float(tol_inner), int(mode),
+                                     _dev(m, self.M, "m"), _dev(dpred, self.N, "dpred"), C.c_void_p(hist.ctypes.data),
+                                     C.c_void_p(steps.ctypes.data), inner, C.byref(n_outer), _stream()))
         k = n_outer.value
         stop = "tolerance" if hist[k] <= tol_outer else ("max_outer" if k == max_outer else "no_decrease")
-        return dict(m=m, dpred=dpred, hist=hist[:k + 1], steps=steps[:k], n_outer=k, stop=stop)
+        tried = min(k + (1 if stop == "no_decrease" else 0), max_outer)
+        return dict(m=m, dpred=dpred, hist=hist[:k + 1], steps=steps[:k], inner=np.array(inner[:tried]), n_outer=k,
+                    stop=stop)
 
     def store_g(self, fp32=False):
         want = STORED_F32 if fp32 else STORED_F64

@@ -547,8 +547,9 @@ grav_status grav_direct_solve(grav_ctx* c, const double* dobs, const double* w, 
 
 // ---- outer model-update loop (csrc/invert.cu has the passage and the readings) -----------------------------
 grav_status grav_invert(grav_ctx* c, const double* dobs, const double* w, double lambda, const double* mref,
-                        int max_outer, int max_inner, double tol_outer, double tol_inner, int mode, double* m,
-                        double* dpred, double* hist_host, double* step_host, int* n_outer_host, void* stream) {
+                        const double* precond, int max_outer, int max_inner, double tol_outer, double tol_inner,
+                        int mode, double* m, double* dpred, double* hist_host, double* step_host, int* inner_host,
+                        int* n_outer_host, void* stream) {
     grav_status st = check_ready(c);
     if (st) return st;
     if (!dobs || !w || !m) return fail(GRAV_EINVAL, "NULL vector");
@@ -596,8 +597,11 @@ grav_status grav_invert(grav_ctx* c, const double* dobs, const double* w, double
     int k = 0;
     for (; k < max_outer; ++k) {
         if (std::sqrt(nr2) / dn <= tol_outer) break;
-        st = grav_dataspace_cg(c, r, w, lambda, max_inner, tol_inner, mode, nullptr, nullptr, alpha, dm, nullptr, nullptr, stream);
+        st = grav_dataspace_cg(c, r, w, lambda, max_inner, tol_inner, mode, precond, nullptr, alpha, dm, nullptr, nullptr, stream);
         if (st) return st;
+        if (inner_host)     // ordered on the stream; read after the first trial's synchronisation
+            CK(cudaMemcpyAsync(inner_host + k, &wsp<CgScalars>(c, c->lay.scalars)->iters_done, sizeof(int),
+                               cudaMemcpyDeviceToHost, s), "D2H inner iterations");
         if ((st = apply_G(dm, dd))) return st;
         double step = 1.0, n2 = 0.0;
         bool ok = false;

@@ -136,7 +136,7 @@ static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev, int zb_sh
     const size_t tab = ev == 0 ? 0 : (ev == 2 ? psi_smem_bytes<true>(pd) : kTabSmemBytes);
     return tab + (size_t)((g.nzp + 1) & ~1) * 8 + (size_t)kPairTPB * ((1 << zb_shift) + 1) * 8;
 }
-constexpr size_t kPairSmemMax = 227 * 1024;
+constexpr size_t kPairSmemMax = 226 * 1024;     // dynamic part: the opt-in limit of 227 KB includes the static s_red
 
 // Tile shape: tnx * tny <= kPairTPB node columns minimising the number of tiles (every tile costs one block the same
 // time), ties towards the squarer tile; batch depth 32 layers, 16 or 8 when the tables leave less shared memory.
