@@ -151,23 +151,39 @@ def test_no_decrease_exit(prob):
 
 def test_inner_tolerance_stop(prob):
     """tol_inner between two consecutive residuals of the first inner solve (oracle.pcg on rhs = d_obs) stops that
-    solve after exactly that iteration; the count is reported and the update equals the oracle's."""
+    solve after exactly that iteration; the count is reported and the update equals the oracle's.
+
+    CG iterates stop being unique to 1e-8 once orthogonality is lost (on this problem from iteration
+    ~8-10), so the cases are the first two iterations that set a new residual minimum, and each is admitted only if
+    the oracle ALONE, run on a G perturbed by 1e-11 (the size of the operator difference between the two codes), moves
+    its own result by < 1e-9: two updates where that holds, otherwise one."""
     G, w, lam, d, ctx, diag = prob["G"], prob["w"], prob["lam"], prob["d"], prob["ctx"], prob["diag"]
+    Gp = G * (1.0 + 1e-11 * np.random.default_rng(5).standard_normal(G.shape))
+    checked = 0
     for dg in (None, diag):
         _, hcg, _, _ = oracle.pcg(G, w, lam, d, 12, diag=dg)
         rel = hcg / hcg[0]
         cand = [j for j in range(11) if rel[j + 1] < rel[:j + 1].min()]      # iterations that set a new minimum
-        assert len(cand) >= 3
-        for j in (cand[1], cand[-1]):
+        assert len(cand) >= 2
+        for j in cand[:2]:
             tol = float(np.sqrt(rel[:j + 1].min() * rel[j + 1]))
-            ref = oracle.invert(G, w, lam, d, max_outer=2, max_inner=12, tol_outer=0.0, tol_inner=tol, diag=dg,
-                                details=True)
+            for max_outer in (2, 1):
+                kw = dict(max_outer=max_outer, max_inner=12, tol_outer=0.0, tol_inner=tol, diag=dg, details=True)
+                ref = oracle.invert(G, w, lam, d, **kw)
+                pert = oracle.invert(Gp, w, lam, d, **kw)
+                if (pert[3].tolist() == ref[3].tolist() and pert[4]["inner"].tolist() == ref[4]["inner"].tolist()
+                        and relmax(pert[0], ref[0]) < 1e-9 and np.abs(pert[2] / ref[2] - 1).max() < 1e-9):
+                    break
+            else:
+                raise AssertionError("the oracle's own result is not unique for this case - pick another")
             assert ref[4]["inner"][0] == j + 1
             for mode in MODES:
-                out = ctx.invert(dev(d), dev(w), lam, max_outer=2, max_inner=12, tol_outer=0.0, tol_inner=tol,
+                out = ctx.invert(dev(d), dev(w), lam, max_outer=max_outer, max_inner=12, tol_outer=0.0, tol_inner=tol,
                                  mode=mode, precond=None if dg is None else dev(dg))
                 assert out["inner"][0] == j + 1
                 compare(out, ref, d, f"inner stop after {j + 1}, precond {dg is not None}, mode {mode}")
+                checked += 1
+    assert checked == 8
 
 
 def test_paper_schedule_runs_to_an_exit(prob):
