@@ -125,10 +125,10 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
     const int kc = c->plan.adj_kc;           // the plan's choice of KC (grav_api.cu make_plan)
     cudaError_t e;
     if (c->psi_variant == 1) e = adj_launch<128, 4, 4, 0>(c, v, partial, done, s);
-    else if (use_log2d(c)) {
+    else if (use_log2d(c)) {      // (threads, KC) pairs of make_plan's table
         if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, s);
-        else if (kc == 5) e = adj_launch<512, 5, 1, 2>(c, v, partial, done, s);
-        else if (kc == 6) e = adj_launch<256, 6, 1, 2>(c, v, partial, done, s);
+        else if (kc == 5) e = adj_launch<384, 5, 1, 2>(c, v, partial, done, s);
+        else if (kc == 6) e = adj_launch<384, 6, 1, 2>(c, v, partial, done, s);
         else e = adj_launch<256, 8, 1, 2>(c, v, partial, done, s);
     } else {
         if (kc == 4) e = adj_launch<256, 4, 2, 1>(c, v, partial, done, s);

@@ -54,19 +54,25 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
     // KC nodes per thread: the per-(thread, station) set-up is shared by KC evaluations but the column is padded to a
-    // multiple of KC.  Measured scheduler cycles per warp-evaluation fit (119.5 + 25.6 / KC) x padding within 1 % for
-    // KC = 4, 5, 6, 8 at configs 3 and 5 (profiles/r1_tail_and_variants.md); pick the cheapest compiled variant.
-    // With the 2-D log table the fit is (108.5 + 32.8 / KC) x padding.
+    // multiple of KC.  With the 2-D log table the compiled (threads, KC) variants measure 114.3 (256, 8), 112.5 (384, 6),
+    // 114.5 (384, 5) and 116.3 (512, 4) scheduler cycles per warp-evaluation before padding (configs 3 and 5,
+    // profiles/r2_adjoint_variants.md); without it the fit of round 1 stands, (119.5 + 25.6 / KC).  Pick the cheapest.
     p.adj_tpb = 256;
     p.adj_kc = 4;
     double best = 1e300;
-    for (int kc : {4, 5, 6, 8}) {
-        const double per_eval = log2d ? 108.5 + 32.8 / kc : 119.5 + 25.6 / kc;
-        const double cost = per_eval * (double)(ceil_div(g.nzp, kc) * kc);
-        if (cost < best) { best = cost; p.adj_kc = kc; }
+    if (log2d) {
+        const struct { int tpb, kc; double cyc; } var[] = {{256, 8, 114.3}, {384, 6, 112.5}, {384, 5, 114.5}, {512, 4, 116.3}};
+        for (const auto& v : var) {
+            const double cost = v.cyc * (double)(ceil_div(g.nzp, v.kc) * v.kc);
+            if (cost < best) { best = cost; p.adj_kc = v.kc; p.adj_tpb = v.tpb; }
+        }
+    } else {
+        for (int kc : {4, 5, 6, 8}) {
+            const double cost = (119.5 + 25.6 / kc) * (double)(ceil_div(g.nzp, kc) * kc);
+            if (cost < best) { best = cost; p.adj_kc = kc; }
+        }
+        p.adj_tpb = p.adj_kc >= 6 ? 128 : 256;
     }
-    if (log2d) p.adj_tpb = p.adj_kc <= 5 ? 512 : 256;
-    else if (p.adj_kc >= 6) p.adj_tpb = 128;
     p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
     p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
     want = ceil_div(log2d ? 148 * 48 : 148 * 128, p.adj_blocks);
@@ -455,7 +461,8 @@ grav_status grav_gram_diag(grav_ctx* c, const double* w, double* diag, void* str
     if (st) return st;
     if (!w || !diag) return fail(GRAV_EINVAL, "NULL argument");
     DeviceGuard dg(c->device);
-    CK(launch_gram_diag(c, w, wsp<double>(c, c->lay.gram_partial), diag, (cudaStream_t)stream), "gram_diag");
+    CK(launch_gram_diag(c, w, wsp<double>(c, c->lay.gcell), wsp<double>(c, c->lay.gram_partial), diag,
+                        (cudaStream_t)stream), "gram_diag");
     return GRAV_OK;
 }
 

@@ -129,7 +129,9 @@ cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s);
 cudaError_t launch_gemv(grav_ctx* c, const void* G, int elem, const double* u, double* d, cudaStream_t s);
 cudaError_t launch_gemvt(grav_ctx* c, const void* G, int elem, const double* v, const double* w_or_null, double* g,
                          double* partial, cudaStream_t s);
-cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* partial, double* diag, cudaStream_t s);
+// winv2: M doubles of scratch (1 / w^2)
+cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* winv2, double* partial, double* diag,
+                             cudaStream_t s);
 cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double lam, double* A, cudaStream_t s);
 cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
 int gemvt_chunks(long long N);

@@ -18,23 +18,31 @@
 namespace grav {
 
 // ---- per-pair evaluation, node-shared --------------------------------------------------------------------
-constexpr int kPairTPB = 320;            // >= 17 x 17 node columns: 16 x 16 cell columns per tile
+constexpr int kPairTPB = 512;            // >= 22 x 23 node columns: 21 x 22 cell columns per tile
+constexpr int kPairWarps = kPairTPB / 32;
 constexpr int kPairU = 8;                // evaluations in flight per thread
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 
-// Work item = (station, tile), tile index fastest; blocks stride over the items.  Phase A: thread t < nnx * nny owns
-// node column (i0 + t / nny, j0 + t % nny): hoists once per item, then Psi down the column in batches of zb layers,
-// storing dPsi(k) = Psi(k+1) - Psi(k) at s_d[t * (zb + 1) + k - k0] (odd stride: conflict-free).  Phase B: entry
-// (li, lj, k) = gamma * ((d11 - d21) - d12 + d22) with lanes along k - the same pairing as node_to_cell (vertical
-// neighbours first: their Psi values are closest), so stored and matrix-free products agree to rounding.
+// Work item = (station, tile), tile index fastest; blocks stride over the items; the z-axis of an item is cut into
+// batches of zb = 2^zb_shift layers.
+// Phase A(batch): thread t < nnx * nny owns node column (i0 + t / nny, j0 + t % nny): hoists once per item, then Psi down
+//   the column, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * (zb + 1) + k - k0] (odd stride: conflict-free).
+// Phase B(batch): entry (li, lj, k) = gamma * ((d11 - d21) - d12 + d22) - the same pairing as node_to_cell (vertical
+//   neighbours first: their Psi values are closest), so stored and matrix-free products agree to rounding.  A warp takes
+//   32 >> zb_shift neighbouring cell columns of one tile row at a time, lanes along k (contiguous in G); which (row, chunk)
+//   a warp takes next is kept incrementally, so there is no division in the loop.
+// The difference buffer is double-buffered: every thread runs A(b), barrier, B(b), A(b+1), barrier, B(b+1), ... - ONE
+// barrier per batch (B(b-1) precedes barrier b in every thread, so buffer (b+1)&1 is free after it), and between two
+// barriers the warps that are still storing entries overlap with the warps that already evaluate the next batch.
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = with the 2-D log table.
+// PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[item].
 template <int MODE, int EV>
 __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev pd, int tnx, int tny, int tiles_y,
                                                                int ntiles, int zb_shift, void* __restrict__ Gout,
-                                                               const double* __restrict__ w,
+                                                               const double* __restrict__ winv2,
                                                                double* __restrict__ gram_partial) {
     extern __shared__ double2 s_tab[];
-    __shared__ double s_red[kPairTPB / 32];
+    __shared__ double s_red[kPairWarps];
     PsiTabView tb;
     size_t tab_entries = 0;
     if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); tab_entries = (size_t)kTabEntries * kRep; }
@@ -43,9 +51,11 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     double* s_d = s_zn + ((g.nzp + 1) & ~1);
     for (int c = threadIdx.x; c < g.nzp; c += kPairTPB) s_zn[c] = g.zn[c];
     __syncthreads();
-    const int zb = 1 << zb_shift, stride = zb + 1;
-    const int t = threadIdx.x;
+    const int zb = 1 << zb_shift, stride = zb + 1, bufsz = kPairTPB * stride;
+    const int t = threadIdx.x, warp = t >> 5;
+    const int l = t & (zb - 1), sub = (t & 31) >> zb_shift, cpw = 32 >> zb_shift;   // phase B: layer, cell within chunk
     const long long nitems = g.N * (long long)ntiles;
+    int par = 0;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const long long st = item / ntiles;
         const int tile = (int)(item - st * ntiles);
@@ -66,12 +76,18 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
             if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
             return pc.s * psi_eval<EV == 2>(tb, pc, Z);
         };
+        // phase B units of this tile: (tile row li, chunk of cpw cell columns); a warp takes units warp, warp + 16, ...
+        const int nchy = (ncy + cpw - 1) / cpw, nunits = ncx * nchy;
+        const int dl = kPairWarps / nchy, dq = kPairWarps - dl * nchy;
+        const int li_first = warp / nchy, ch_first = warp - li_first * nchy;
+        const long long row = st * g.M;
         double prev = active ? eval(0) : 0.0;
         double gram = 0.0;
-        for (int k0 = 0; k0 < g.nz; k0 += zb) {
+        for (int k0 = 0; k0 < g.nz; k0 += zb, par ^= 1) {
             const int nb = min(zb, g.nz - k0);
+            double* buf = s_d + par * bufsz;
             if (active) {
-                double* dst = s_d + t * stride;
+                double* dst = buf + t * stride;
                 // kPairU independent evaluations in flight; layers past the mesh bottom (last partial group only) are
                 // evaluated at the bottom layer and dropped
                 for (int kk = 0; kk < nb; kk += kPairU) {
@@ -87,39 +103,41 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 }
             }
             __syncthreads();
-            // phase B: flattened (cell column, layer) pairs, layer fastest
-            const int nent = (ncx * ncy) << zb_shift;
-            for (int e = t; e < nent; e += kPairTPB) {
-                const int cc = e >> zb_shift, l = e & (zb - 1);
-                if (l >= nb) continue;
-                const int li = cc / ncy, lj = cc - li * ncy;
-                const double* d11 = s_d + (li * nny + lj) * stride + l;
-                const double* d21 = d11 + nny * stride;
-                const double val = g.gamma * (((d11[0] - d21[0]) - d11[stride]) + d21[stride]);
-                const long long cell = ((long long)(i0 + li) * g.ny + (j0 + lj)) * g.nz + k0 + l;
-                if (MODE == PAIR_F64) reinterpret_cast<double*>(Gout)[st * g.M + cell] = val;
-                else if (MODE == PAIR_F32) reinterpret_cast<float*>(Gout)[st * g.M + cell] = (float)val;
-                else {
-                    const double q = val / w[cell];
-                    gram = fma(q, q, gram);
+            int li = li_first, ch = ch_first;
+            for (int unit = warp; unit < nunits; unit += kPairWarps) {
+                const int lj = ch * cpw + sub;
+                if (lj < ncy && l < nb) {
+                    const double* d11 = buf + (li * nny + lj) * stride + l;
+                    const double* d21 = d11 + nny * stride;
+                    const double val = g.gamma * (((d11[0] - d21[0]) - d11[stride]) + d21[stride]);
+                    const long long cell = ((long long)(i0 + li) * g.ny + (j0 + lj)) * g.nz + k0 + l;
+                    if (MODE == PAIR_F64) reinterpret_cast<double*>(Gout)[row + cell] = val;
+                    else if (MODE == PAIR_F32) reinterpret_cast<float*>(Gout)[row + cell] = (float)val;
+                    else gram = fma(val * val, winv2[cell], gram);
                 }
+                li += dl; ch += dq;
+                if (ch >= nchy) { ch -= nchy; ++li; }
             }
-            __syncthreads();
         }
         if (MODE == PAIR_GRAM) {      // fixed-order block sum -> gram_partial[station][tile]
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) gram += __shfl_down_sync(0xffffffffu, gram, o);
-            if ((t & 31) == 0) s_red[t >> 5] = gram;
+            if ((t & 31) == 0) s_red[warp] = gram;
             __syncthreads();
             if (t == 0) {
                 double sum = 0.0;
 #pragma unroll
-                for (int k = 0; k < kPairTPB / 32; ++k) sum += s_red[k];
+                for (int k = 0; k < kPairWarps; ++k) sum += s_red[k];
                 gram_partial[item] = sum;
             }
             __syncthreads();
         }
     }
+}
+
+__global__ void gram_winv2_kernel(long long M, const double* __restrict__ w, double* __restrict__ winv2) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m < M) { const double ww = w[m]; winv2[m] = 1.0 / (ww * ww); }
 }
 
 // diag[st] = sum over tiles of gram_partial[st][tile], in tile order
@@ -134,12 +152,13 @@ __global__ void gram_reduce_kernel(long long N, int ntiles, const double* __rest
 
 static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev, int zb_shift) {
     const size_t tab = ev == 0 ? 0 : (ev == 2 ? psi_smem_bytes<true>(pd) : kTabSmemBytes);
-    return tab + (size_t)((g.nzp + 1) & ~1) * 8 + (size_t)kPairTPB * ((1 << zb_shift) + 1) * 8;
+    return tab + (size_t)((g.nzp + 1) & ~1) * 8 + 2 * (size_t)kPairTPB * ((1 << zb_shift) + 1) * 8;   // double-buffered
 }
 constexpr size_t kPairSmemMax = 226 * 1024;     // dynamic part: the opt-in limit of 227 KB includes the static s_red
 
 // Tile shape: tnx * tny <= kPairTPB node columns minimising the number of tiles (every tile costs one block the same
-// time), ties towards the squarer tile; batch depth 32 layers, 16 or 8 when the tables leave less shared memory.
+// time), ties towards the squarer tile; batch depth 32 layers, 16 or 8 when the tables leave less shared memory (8 with
+// the 2-D log table of the five configs).
 void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     long long best = -1;
     p.pair_tnx = p.pair_tny = 2;
@@ -358,12 +377,14 @@ cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s) {
     return e;
 }
 
-cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* partial, double* diag, cudaStream_t s) {
-    cudaError_t e = pair_dispatch<PAIR_GRAM>(c, nullptr, w, partial, s);
+cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* winv2, double* partial, double* diag,
+                             cudaStream_t s) {
+    gram_winv2_kernel<<<(unsigned)((c->g.M + 255) / 256), 256, 0, s>>>(c->g.M, w, winv2);
+    cudaError_t e = pair_dispatch<PAIR_GRAM>(c, nullptr, winv2, partial, s);
     if (e != cudaSuccess) return e;
     gram_reduce_kernel<<<(unsigned)((c->g.N + 255) / 256), 256, 0, s>>>(c->g.N, c->plan.pair_tiles_x * c->plan.pair_tiles_y,
                                                                         partial, diag);
-    c->launches += 2;
+    c->launches += 3;
     return cudaGetLastError();
 }
 
