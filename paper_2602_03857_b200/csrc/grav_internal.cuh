@@ -33,7 +33,7 @@ struct Plan {
     // adjoint: grid (node-thread blocks, station chunks)
     int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;
     // per-pair family (stored.cu): node tile of pair_tnx x pair_tny node columns per block
-    int pair_tnx, pair_tny, pair_tiles_x, pair_tiles_y, pair_zb_shift;
+    int pair_tnx, pair_tny, pair_tiles_x, pair_tiles_y;
 };
 
 constexpr int kDotBlocks = 256;     // block partials of the fused CG dot products

@@ -21,24 +21,33 @@ namespace grav {
 constexpr int kPairTPB = 512;            // >= 22 x 23 node columns: 21 x 22 cell columns per tile
 constexpr int kPairWarps = kPairTPB / 32;
 constexpr int kPairU = 8;                // evaluations in flight per thread
+constexpr int kPairZPad = 32;             // bottom node repeated this many times behind the node depths in shared memory
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
+__host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPairZPad + 1) & ~1; }
 
 // Work item = (station, tile), tile index fastest; blocks stride over the items; the z-axis of an item is cut into
-// batches of zb = 2^zb_shift layers.
+// batches of zb layers.
 // Phase A(batch): thread t < nnx * nny owns node column (i0 + t / nny, j0 + t % nny): hoists once per item, then Psi down
-//   the column, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * (zb + 1) + k - k0] (odd stride: conflict-free).
-// Phase B(batch): entry (li, lj, k) = gamma * ((d11 - d21) - d12 + d22) - the same pairing as node_to_cell (vertical
-//   neighbours first: their Psi values are closest), so stored and matrix-free products agree to rounding.  A warp takes
-//   32 >> zb_shift neighbouring cell columns of one tile row at a time, lanes along k (contiguous in G); which (row, chunk)
-//   a warp takes next is kept incrementally, so there is no division in the loop.
-// The difference buffer is double-buffered: every thread runs A(b), barrier, B(b), A(b+1), barrier, B(b+1), ... - ONE
-// barrier per batch (B(b-1) precedes barrier b in every thread, so buffer (b+1)&1 is free after it), and between two
-// barriers the warps that are still storing entries overlap with the warps that already evaluate the next batch.
+//   the column, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * stride + k - k0] (stride = zb + 2 doubles: 16-byte aligned
+//   rows whose 16-byte bank groups differ between neighbouring threads - conflict-free 128-bit accesses).
+// Phase B(batch): the thread of node column (la, lb) with la < ncx, lb < ncy also owns CELL column (la, lb): its zb
+//   entries are gamma * ((d11 - d21) - d12 + d22) from its own row of the buffer and the rows of threads t + 1, t + nny,
+//   t + nny + 1 - the same pairing as node_to_cell (vertical neighbours first: their Psi values are closest), so stored
+//   and matrix-free products agree to rounding.  zb independent entries per thread (no dependent chain), written as
+//   16-byte vector stores: every lane fills whole 32-byte sectors of its own prism column.
+// The difference buffer is double-buffered: every thread runs A(0), then per batch b: barrier, B(b) and A(b+1) - ONE
+// barrier per batch (B(b-1) precedes barrier b in every thread, so buffer (b+1)&1 is free after it).  Even warps run
+// B(b) first, odd warps A(b+1) first: the entry stores of one half overlap the FP64 work of the other.
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = with the 2-D log table.
-// PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[item].
+// PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[station][tile].
+
+// Batch depth: 8 layers beside the 2-D log table (92-110 KB at the configs), 16 otherwise; compile-time so that the
+// entries of a thread live in registers.
+template <int EV> constexpr int pair_zb() { return EV == 2 ? 8 : 16; }
+
 template <int MODE, int EV>
 __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev pd, int tnx, int tny, int tiles_y,
-                                                               int ntiles, int zb_shift, void* __restrict__ Gout,
+                                                               int ntiles, void* __restrict__ Gout,
                                                                const double* __restrict__ winv2,
                                                                double* __restrict__ gram_partial) {
     extern __shared__ double2 s_tab[];
@@ -48,75 +57,129 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); tab_entries = (size_t)kTabEntries * kRep; }
     if (EV == 2) { tb = psi_tables_to_smem_2d(s_tab, pd); tab_entries = psi_log2d_smem_entries(pd); }
     double* s_zn = reinterpret_cast<double*>(s_tab + tab_entries);
-    double* s_d = s_zn + ((g.nzp + 1) & ~1);
-    for (int c = threadIdx.x; c < g.nzp; c += kPairTPB) s_zn[c] = g.zn[c];
+    double* s_d = s_zn + pair_zn_doubles(g.nzp);
+    // node depths, the bottom node repeated so that phase A never has to clamp an index past the mesh bottom
+    for (int c = threadIdx.x; c < g.nzp + kPairZPad; c += kPairTPB) s_zn[c] = g.zn[min(c, g.nz)];
     __syncthreads();
-    const int zb = 1 << zb_shift, stride = zb + 1, bufsz = kPairTPB * stride;
+    constexpr int zb = pair_zb<EV>(), stride = zb + 2, bufsz = kPairTPB * stride;
+    static_assert(zb % kPairU == 0 && kPairZPad >= zb, "batch = whole groups of evaluations; padding covers a batch");
     const int t = threadIdx.x, warp = t >> 5;
-    const int l = t & (zb - 1), sub = (t & 31) >> zb_shift, cpw = 32 >> zb_shift;   // phase B: layer, cell within chunk
-    const long long nitems = g.N * (long long)ntiles;
+    const int ds = (int)(gridDim.x / ntiles), dt = (int)(gridDim.x - ds * ntiles);  // item += gridDim.x as (station, tile)
+    // 16-byte vector stores / loads need the prism columns 16-byte aligned in G: nz a multiple of 4 (FP32) or 2 (FP64)
+    const bool vec_ok = MODE == PAIR_F32 ? (g.nz & 3) == 0 : (g.nz & 1) == 0;
+    long long st = blockIdx.x / ntiles;
+    int tile = (int)(blockIdx.x - st * ntiles);
     int par = 0;
-    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const long long st = item / ntiles;
-        const int tile = (int)(item - st * ntiles);
+    for (; st < g.N; st += ds, tile += dt) {
+        if (tile >= ntiles) { tile -= ntiles; if (++st >= g.N) break; }
         const int tx = tile / tiles_y, ty = tile - tx * tiles_y;
         const int i0 = tx * (tnx - 1), j0 = ty * (tny - 1);
         const int nnx = min(tnx, g.nxp - i0), nny = min(tny, g.nyp - j0);       // node columns of this tile
-        const int ncx = nnx - 1, ncy = nny - 1;                                 // cell columns of this tile
         const bool active = t < nnx * nny;
         const int la = active ? t / nny : 0, lb = active ? t - la * nny : 0;
+        const bool owns_cell = active && la < nnx - 1 && lb < nny - 1;          // cell column (la, lb) of this tile
         const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
         const double X = g.xn[i0 + la] - xo, Y = g.yn[j0 + lb] - yo;
         PsiColumn pc;
         double XY = 0.0, Q = 0.0;
         if (EV != 0) pc = psi_column(X, Y);
         else { XY = X * Y; Q = fma(Y, Y, X * X); }
-        auto eval = [&](int c) -> double {
-            const double Z = s_zn[c] - zo;
+        auto eval = [&](double zn) -> double {
+            const double Z = zn - zo;
             if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
             return pc.s * psi_eval<EV == 2>(tb, pc, Z);
         };
-        // phase B units of this tile: (tile row li, chunk of cpw cell columns); a warp takes units warp, warp + 16, ...
-        const int nchy = (ncy + cpw - 1) / cpw, nunits = ncx * nchy;
-        const int dl = kPairWarps / nchy, dq = kPairWarps - dl * nchy;
-        const int li_first = warp / nchy, ch_first = warp - li_first * nchy;
-        const long long row = st * g.M;
-        double prev = active ? eval(0) : 0.0;
+        const int d21 = nny * stride;
+        // first entry of this thread's prism column in this station's row of G (element index fits 63 bits; the row
+        // base is kept opaque so that the compiler does not re-form st * M per store)
+        const int cell_first = ((i0 + la) * g.ny + j0 + lb) * g.nz;
+        size_t Grow = (size_t)Gout + (size_t)st * (size_t)g.M * (MODE == PAIR_F64 ? 8 : 4);
+        asm volatile("" : "+l"(Grow));
+        double prev = active ? eval(s_zn[0]) : 0.0;
         double gram = 0.0;
-        for (int k0 = 0; k0 < g.nz; k0 += zb, par ^= 1) {
+        auto phase_a = [&](int k0, double* buf) {
+            if (!active) return;
             const int nb = min(zb, g.nz - k0);
-            double* buf = s_d + par * bufsz;
-            if (active) {
-                double* dst = buf + t * stride;
-                // kPairU independent evaluations in flight; layers past the mesh bottom (last partial group only) are
-                // evaluated at the bottom layer and dropped
-                for (int kk = 0; kk < nb; kk += kPairU) {
-                    double cur[kPairU];
+            double* dst = buf + t * stride;
+            // kPairU independent evaluations in flight; layers past the mesh bottom (last partial group only) are
+            // evaluated at the bottom node (s_zn is padded), stored, and never used
+            for (int kk = 0; kk < nb; kk += kPairU) {
+                const double* zp = s_zn + k0 + kk + 1;
+                double cur[kPairU];
 #pragma unroll
-                    for (int u = 0; u < kPairU; ++u) cur[u] = eval(min(k0 + kk + u + 1, g.nz));
-                    double last = prev;
+                for (int u = 0; u < kPairU; ++u) cur[u] = eval(zp[u]);
 #pragma unroll
-                    for (int u = 0; u < kPairU; ++u) {
-                        if (kk + u < nb) { dst[kk + u] = cur[u] - last; prev = cur[u]; }
-                        last = cur[u];
+                for (int u = 0; u < kPairU; u += 2)
+                    *reinterpret_cast<double2*>(dst + kk + u) =
+                        make_double2(cur[u] - (u ? cur[u - 1] : prev), cur[u + 1] - cur[u]);
+                prev = cur[kPairU - 1];
+            }
+        };
+        auto phase_b = [&](int k0, const double* buf) {
+            if (!owns_cell) return;
+            const int nb = min(zb, g.nz - k0);
+            const double* p11 = buf + t * stride;
+            double val[zb];
+#pragma unroll
+            for (int u = 0; u < zb; u += 2) {
+                const double2 a = *reinterpret_cast<const double2*>(p11 + u);
+                const double2 b = *reinterpret_cast<const double2*>(p11 + d21 + u);
+                const double2 c = *reinterpret_cast<const double2*>(p11 + stride + u);
+                const double2 d = *reinterpret_cast<const double2*>(p11 + d21 + stride + u);
+                val[u] = g.gamma * (((a.x - b.x) - c.x) + d.x);
+                val[u + 1] = g.gamma * (((a.y - b.y) - c.y) + d.y);
+            }
+            const int cell = cell_first + k0;
+            if (MODE == PAIR_GRAM) {
+                if (nb == zb && vec_ok) {
+#pragma unroll
+                    for (int u = 0; u < zb; u += 2) {
+                        const double2 wi = __ldg(reinterpret_cast<const double2*>(winv2 + cell + u));
+                        gram = fma(val[u] * val[u], wi.x, gram);
+                        gram = fma(val[u + 1] * val[u + 1], wi.y, gram);
                     }
+                } else {
+#pragma unroll
+                    for (int u = 0; u < zb; ++u)
+                        if (u < nb) gram = fma(val[u] * val[u], __ldg(winv2 + cell + u), gram);
+                }
+            } else if (MODE == PAIR_F64) {
+                // (the opaque row address no longer tells the compiler its state space: say st.global)
+                const size_t a0 = Grow + (size_t)cell * 8;
+                if (nb == zb && vec_ok) {
+#pragma unroll
+                    for (int u = 0; u < zb; u += 2)
+                        asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(a0 + u * 8), "d"(val[u]), "d"(val[u + 1]));
+                } else {
+#pragma unroll
+                    for (int u = 0; u < zb; ++u)
+                        if (u < nb) asm volatile("st.global.f64 [%0], %1;" ::"l"(a0 + u * 8), "d"(val[u]));
+                }
+            } else {
+                const size_t a0 = Grow + (size_t)cell * 4;
+                if (nb == zb && vec_ok) {
+#pragma unroll
+                    for (int u = 0; u < zb; u += 4)
+                        asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(a0 + u * 4), "f"((float)val[u]),
+                                     "f"((float)val[u + 1]), "f"((float)val[u + 2]), "f"((float)val[u + 3]));
+                } else {
+#pragma unroll
+                    for (int u = 0; u < zb; ++u)
+                        if (u < nb) asm volatile("st.global.f32 [%0], %1;" ::"l"(a0 + u * 4), "f"((float)val[u]));
                 }
             }
+        };
+        const int nbatch = (g.nz + zb - 1) / zb;
+        phase_a(0, s_d + par * bufsz);
+        for (int b = 0; b < nbatch; ++b, par ^= 1) {
             __syncthreads();
-            int li = li_first, ch = ch_first;
-            for (int unit = warp; unit < nunits; unit += kPairWarps) {
-                const int lj = ch * cpw + sub;
-                if (lj < ncy && l < nb) {
-                    const double* d11 = buf + (li * nny + lj) * stride + l;
-                    const double* d21 = d11 + nny * stride;
-                    const double val = g.gamma * (((d11[0] - d21[0]) - d11[stride]) + d21[stride]);
-                    const long long cell = ((long long)(i0 + li) * g.ny + (j0 + lj)) * g.nz + k0 + l;
-                    if (MODE == PAIR_F64) reinterpret_cast<double*>(Gout)[row + cell] = val;
-                    else if (MODE == PAIR_F32) reinterpret_cast<float*>(Gout)[row + cell] = (float)val;
-                    else gram = fma(val * val, winv2[cell], gram);
-                }
-                li += dl; ch += dq;
-                if (ch >= nchy) { ch -= nchy; ++li; }
+            double* cur = s_d + par * bufsz;
+            double* nxt = s_d + (par ^ 1) * bufsz;
+            const bool more = b + 1 < nbatch;
+#pragma unroll 1
+            for (int ph = 0; ph < 2; ++ph) {
+                if ((ph == 0) == ((warp & 1) != 0)) { if (more) phase_a((b + 1) * zb, nxt); }
+                else phase_b(b * zb, cur);
             }
         }
         if (MODE == PAIR_GRAM) {      // fixed-order block sum -> gram_partial[station][tile]
@@ -128,7 +191,7 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 double sum = 0.0;
 #pragma unroll
                 for (int k = 0; k < kPairWarps; ++k) sum += s_red[k];
-                gram_partial[item] = sum;
+                gram_partial[st * ntiles + tile] = sum;
             }
             __syncthreads();
         }
@@ -150,15 +213,15 @@ __global__ void gram_reduce_kernel(long long N, int ntiles, const double* __rest
     diag[st] = s;
 }
 
-static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev, int zb_shift) {
+static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev) {
+    const int zb = ev == 2 ? pair_zb<2>() : pair_zb<1>();
     const size_t tab = ev == 0 ? 0 : (ev == 2 ? psi_smem_bytes<true>(pd) : kTabSmemBytes);
-    return tab + (size_t)((g.nzp + 1) & ~1) * 8 + 2 * (size_t)kPairTPB * ((1 << zb_shift) + 1) * 8;   // double-buffered
+    return tab + (size_t)pair_zn_doubles(g.nzp) * 8 + 2 * (size_t)kPairTPB * (zb + 2) * 8;   // double-buffered
 }
 constexpr size_t kPairSmemMax = 226 * 1024;     // dynamic part: the opt-in limit of 227 KB includes the static s_red
 
 // Tile shape: tnx * tny <= kPairTPB node columns minimising the number of tiles (every tile costs one block the same
-// time), ties towards the squarer tile; batch depth 32 layers, 16 or 8 when the tables leave less shared memory (8 with
-// the 2-D log table of the five configs).
+// time), ties towards the squarer tile.
 void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     long long best = -1;
     p.pair_tnx = p.pair_tny = 2;
@@ -172,8 +235,6 @@ void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     }
     p.pair_tiles_x = (g.nx + p.pair_tnx - 2) / (p.pair_tnx - 1);
     p.pair_tiles_y = (g.ny + p.pair_tny - 2) / (p.pair_tny - 1);
-    p.pair_zb_shift = 5;
-    while (p.pair_zb_shift > 3 && pair_smem_bytes(g, pd, log2d ? 2 : 1, p.pair_zb_shift) > kPairSmemMax) --p.pair_zb_shift;
 }
 
 size_t gram_partial_doubles(const Geom& g, const Plan& p) { return (size_t)g.N * p.pair_tiles_x * p.pair_tiles_y; }
@@ -181,8 +242,9 @@ size_t gram_partial_doubles(const Geom& g, const Plan& p) { return (size_t)g.N *
 template <int MODE, int EV>
 static cudaError_t pair_launch(grav_ctx* c, void* G, const double* w, double* gram_partial, cudaStream_t s) {
     const Plan& p = c->plan;
-    const size_t smem = pair_smem_bytes(c->g, c->pd, EV, p.pair_zb_shift);
+    const size_t smem = pair_smem_bytes(c->g, c->pd, EV);
     if (smem > kPairSmemMax) return cudaErrorInvalidValue;          // node columns deeper than ~20,000 layers
+    if (c->g.M >= (1ll << 31)) return cudaErrorInvalidValue;        // the kernel keeps cell indices in 32 bits
     static unsigned long long smem_set = 0;
     cudaError_t e = ensure_dynamic_smem(pair_tile_kernel<MODE, EV>, kPairSmemMax, c->device, &smem_set);
     if (e != cudaSuccess) return e;
@@ -192,7 +254,7 @@ static cudaError_t pair_launch(grav_ctx* c, void* G, const double* w, double* gr
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) sms = 148;
     const unsigned blocks = (unsigned)(nitems < sms ? nitems : sms);    // one resident block per SM (shared memory)
     pair_tile_kernel<MODE, EV><<<blocks, kPairTPB, smem, s>>>(c->g, c->pd, p.pair_tnx, p.pair_tny, p.pair_tiles_y,
-                                                               ntiles, p.pair_zb_shift, G, w, gram_partial);
+                                                               ntiles, G, w, gram_partial);
     return cudaGetLastError();
 }
 
@@ -200,7 +262,7 @@ template <int MODE>
 static cudaError_t pair_dispatch(grav_ctx* c, void* G, const double* w, double* gram_partial, cudaStream_t s) {
     if (c->psi_variant == 1) return pair_launch<MODE, 0>(c, G, w, gram_partial, s);
     // the 2-D log table only when it leaves room for the tile buffer
-    if (use_log2d(c) && pair_smem_bytes(c->g, c->pd, 2, c->plan.pair_zb_shift) <= kPairSmemMax)
+    if (use_log2d(c) && pair_smem_bytes(c->g, c->pd, 2) <= kPairSmemMax)
         return pair_launch<MODE, 2>(c, G, w, gram_partial, s);
     return pair_launch<MODE, 1>(c, G, w, gram_partial, s);
 }
