@@ -22,68 +22,85 @@ namespace grav {
 constexpr int kAdjObsTile = 256;
 
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table
+// work != NULL: persistent launch for small problems (see forward.cu): the block fills the tables once and draws
+// (node-thread block, station chunk) items from the counter.
 template <int TPB, int KC, int MINB, int EV>
 __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
                                                                   double* __restrict__ partial, int ncg,
-                                                                  int obs_per_chunk, const int* __restrict__ done) {
+                                                                  int obs_per_chunk, const int* __restrict__ done,
+                                                                  int* __restrict__ work, int nblocks, int nitems) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
+    __shared__ int s_item;
     PsiTabView tb;
     if (EV != 0) tb = psi_tables_load<EV == 2>(s_tab, pd);
-    const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long nthreads = (long long)g.ncol * ncg;
-    const bool valid = t < nthreads;
-    const long long tl = valid ? t : nthreads - 1;
-    const int cg = (int)(tl / g.ncol);        // column index fastest: lanes of a warp are neighbouring columns
-    const int col = (int)(tl - (long long)cg * g.ncol);
-    const int a = col / g.nyp, b = col - a * g.nyp;
-    const int c0 = cg * KC;
-    const double xa = g.xn[a], yb = g.yn[b];
-    double zc[KC], acc[KC];
-#pragma unroll
-    for (int k = 0; k < KC; ++k) {
-        zc[k] = g.zn[min(c0 + k, g.nzp - 1)];
-        acc[k] = 0.0;
-    }
-    const long long i0 = (long long)blockIdx.y * obs_per_chunk;
-    const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
-    double* out_hi = partial + (long long)blockIdx.y * 2 * g.Nn + (long long)col * g.nzp + c0;
-    double* out_lo = out_hi + g.Nn;
-    for (long long base = i0; base < i1; base += kAdjObsTile) {
-        const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
-        __syncthreads();
-        for (int j = threadIdx.x; j < cnt; j += TPB)
-            s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
-        __syncthreads();
-        for (int j = 0; j < cnt; ++j) {
-            const double4 o = s_obs[j];
-            const double X = xa - o.x, Y = yb - o.y;
-            if (EV != 0) {
-                const PsiColumn pc = psi_column(X, Y);
-                const double vs = o.w * pc.s;
-#pragma unroll
-                for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
-            } else {
-                const double XY = X * Y;
-                const double Q = fma(Y, Y, X * X);
-#pragma unroll
-                for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
-            }
+    for (;;) {
+        int bx = blockIdx.x, by = blockIdx.y;
+        if (work) {
+            __syncthreads();                             // the previous item's s_item is done with
+            if (threadIdx.x == 0) s_item = atomicAdd(work, 1);
+            __syncthreads();
+            const int item = s_item;
+            if (item >= nitems) break;
+            by = item / nblocks;                         // node block fastest: neighbours in time share a station chunk
+            bx = item - by * nblocks;
         }
-        // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
-        if (valid) {
+        const long long t = (long long)bx * TPB + threadIdx.x;
+        const bool valid = t < nthreads;
+        const long long tl = valid ? t : nthreads - 1;
+        const int cg = (int)(tl / g.ncol);        // column index fastest: lanes of a warp are neighbouring columns
+        const int col = (int)(tl - (long long)cg * g.ncol);
+        const int a = col / g.nyp, b = col - a * g.nyp;
+        const int c0 = cg * KC;
+        const double xa = g.xn[a], yb = g.yn[b];
+        double zc[KC], acc[KC];
 #pragma unroll
-            for (int k = 0; k < KC; ++k) {
-                if (c0 + k < g.nzp) {
-                    double hi = acc[k], lo = 0.0;
-                    if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
-                    out_hi[k] = hi;
-                    out_lo[k] = lo;
+        for (int k = 0; k < KC; ++k) {
+            zc[k] = g.zn[min(c0 + k, g.nzp - 1)];
+            acc[k] = 0.0;
+        }
+        const long long i0 = (long long)by * obs_per_chunk;
+        const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
+        double* out_hi = partial + (long long)by * 2 * g.Nn + (long long)col * g.nzp + c0;
+        double* out_lo = out_hi + g.Nn;
+        for (long long base = i0; base < i1; base += kAdjObsTile) {
+            const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
+            __syncthreads();
+            for (int j = threadIdx.x; j < cnt; j += TPB)
+                s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
+            __syncthreads();
+            for (int j = 0; j < cnt; ++j) {
+                const double4 o = s_obs[j];
+                const double X = xa - o.x, Y = yb - o.y;
+                if (EV != 0) {
+                    const PsiColumn pc = psi_column(X, Y);
+                    const double vs = o.w * pc.s;
+#pragma unroll
+                    for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
+                } else {
+                    const double XY = X * Y;
+                    const double Q = fma(Y, Y, X * X);
+#pragma unroll
+                    for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
                 }
-                acc[k] = 0.0;
+            }
+            // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
+            if (valid) {
+#pragma unroll
+                for (int k = 0; k < KC; ++k) {
+                    if (c0 + k < g.nzp) {
+                        double hi = acc[k], lo = 0.0;
+                        if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
+                        out_hi[k] = hi;
+                        out_lo[k] = lo;
+                    }
+                    acc[k] = 0.0;
+                }
             }
         }
+        if (!work) break;
     }
 }
 
@@ -94,17 +111,29 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= Nn) return;
     double hi = partial[n], lo = partial[Nn + n];
-    for (int ch = 1; ch < nchunk; ++ch) {
-        const double* pc = partial + (long long)ch * 2 * Nn;
-        two_sum_acc(hi, lo, pc[n], hi, lo);
-        lo += pc[Nn + n];
+    constexpr int U = 8;          // the loads of U chunks are issued together, the TwoSum chain follows in chunk order
+    for (int ch0 = 1; ch0 < nchunk; ch0 += U) {
+        double h[U], l[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double* pc = partial + (long long)min(ch0 + u, nchunk - 1) * 2 * Nn;
+            h[u] = pc[n];
+            l[u] = pc[Nn + n];
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (ch0 + u < nchunk) {
+                two_sum_acc(hi, lo, h[u], hi, lo);
+                lo += l[u];
+            }
     }
     tnode[n] = hi;
     tnode[Nn + n] = lo;
 }
 
 template <int TPB, int KC, int MINB, int EV>
-static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
+static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, const int* done, int* work,
+                              cudaStream_t s) {
     // the opt-in is sized for the largest 2-D table, the launch for this context's table
     const size_t smem = EV == 0 ? 0 : psi_smem_bytes<EV == 2>(c->pd);
     static unsigned long long smem_set = 0;
@@ -115,26 +144,38 @@ static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, con
     }
     const int ncg = (c->g.nzp + KC - 1) / KC;
     const long long nthreads = (long long)c->g.ncol * ncg;
-    dim3 grid((unsigned)((nthreads + TPB - 1) / TPB), c->plan.adj_nchunk);
+    const int nblocks = (int)((nthreads + TPB - 1) / TPB);
+    const long long nitems = (long long)nblocks * c->plan.adj_nchunk;
+    dim3 grid((unsigned)nblocks, c->plan.adj_nchunk);
+    if (c->plan.persistent && EV != 0 && nitems < (1ll << 31)) {
+        cudaError_t e = cudaMemsetAsync(work, 0, sizeof(int), s);
+        if (e != cudaSuccess) return e;
+        const long long resident = (long long)c->plan.sms * MINB;
+        grid = dim3((unsigned)(nitems < resident ? nitems : resident), 1);
+    } else {
+        work = nullptr;
+    }
     adjoint_nodes_kernel<TPB, KC, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, v, partial, ncg,
-                                                                    c->plan.adj_obs_per_chunk, done);
+                                                                    c->plan.adj_obs_per_chunk, done, work, nblocks,
+                                                                    (int)nitems);
     return cudaGetLastError();
 }
 
-cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s) {
+cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, int* work,
+                                 cudaStream_t s) {
     const int kc = c->plan.adj_kc;           // the plan's choice of KC (grav_api.cu make_plan)
     cudaError_t e;
-    if (c->psi_variant == 1) e = adj_launch<128, 4, 4, 0>(c, v, partial, done, s);
+    if (c->psi_variant == 1) e = adj_launch<128, 4, 4, 0>(c, v, partial, done, work, s);
     else if (use_log2d(c)) {      // (threads, KC) pairs of make_plan's table
-        if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, s);
-        else if (kc == 5) e = adj_launch<384, 5, 1, 2>(c, v, partial, done, s);
-        else if (kc == 6) e = adj_launch<384, 6, 1, 2>(c, v, partial, done, s);
-        else e = adj_launch<256, 8, 1, 2>(c, v, partial, done, s);
+        if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, work, s);
+        else if (kc == 5) e = adj_launch<384, 5, 1, 2>(c, v, partial, done, work, s);
+        else if (kc == 6) e = adj_launch<384, 6, 1, 2>(c, v, partial, done, work, s);
+        else e = adj_launch<256, 8, 1, 2>(c, v, partial, done, work, s);
     } else {
-        if (kc == 4) e = adj_launch<256, 4, 2, 1>(c, v, partial, done, s);
-        else if (kc == 5) e = adj_launch<256, 5, 2, 1>(c, v, partial, done, s);
-        else if (kc == 6) e = adj_launch<128, 6, 3, 1>(c, v, partial, done, s);
-        else e = adj_launch<128, 8, 2, 1>(c, v, partial, done, s);
+        if (kc == 4) e = adj_launch<256, 4, 2, 1>(c, v, partial, done, work, s);
+        else if (kc == 5) e = adj_launch<256, 5, 2, 1>(c, v, partial, done, work, s);
+        else if (kc == 6) e = adj_launch<128, 6, 3, 1>(c, v, partial, done, work, s);
+        else e = adj_launch<128, 8, 2, 1>(c, v, partial, done, work, s);
     }
     c->launches++;
     return e;

@@ -5,7 +5,7 @@
 //     q = A p;  delta = p.q;  a = rho/delta;  x += a p;  r -= a q;  z = M^-1 r;  rho' = r.z;  b = rho'/rho;  p = z + b p.
 // Without a preconditioner z IS r (the same buffer) and rho = r.r.  All scalars stay on the device (CgScalars); dot
 // products are two-stage with a fixed tree order, every block re-reduces the same kDotBlocks partials, so all blocks see
-// bit-identical scalars and the result is deterministic.  q = G(.) + lambda p and the p.q partials are produced by
+// bit-identical scalars and the result is deterministic.  rho and the frozen flag are double-buffered by iteration parity.  q = G(.) + lambda p and the p.q partials are produced by
 // forward_reduce (forward.cu) or dot_pq (stored-G mode).  Dot partial layout: [A: p.q | B: r.z | C: r.r].
 #include "grav_internal.cuh"
 
@@ -76,9 +76,9 @@ __global__ void __launch_bounds__(kDotThreads) cg_init_finish_kernel(const doubl
         sc->tol2 = rtol * rtol * dn2;
         sc->delta = 0.0; sc->a = 0.0; sc->b = 0.0;
         sc->rr = rr;
-        sc->done = (rtol > 0.0 && rr <= sc->tol2) ? 1 : 0;
+        sc->done[0] = (rtol > 0.0 && rr <= sc->tol2) ? 1 : 0;
+        sc->done[1] = 0;
         sc->iters_done = 0;
-        sc->it = 0;
         if (hist) hist[0] = sqrt(rr);
     }
 }
@@ -109,14 +109,15 @@ __global__ void __launch_bounds__(kDotThreads) cg_update_xr_kernel(long long N, 
                                                                     const double* __restrict__ q,
                                                                     const double* __restrict__ minv, double lam,
                                                                     double* z, const double* __restrict__ dotp_in,
-                                                                    double* __restrict__ dotp_out, CgScalars* sc) {
-    if (sc->done) {
+                                                                    double* __restrict__ dotp_out, CgScalars* sc,
+                                                                    int it) {
+    if (sc->done[it & 1]) {
         if (threadIdx.x == 0) { dotp_out[blockIdx.x] = 0.0; dotp_out[kDotBlocks + blockIdx.x] = 0.0; }
         return;
     }
     __shared__ double sh[kDotThreads];
     const double delta = sum_partials(dotp_in, sh);
-    const double a = sc->rho[sc->it & 1] / delta;
+    const double a = sc->rho[it & 1] / delta;
     double loc = 0.0, locz = 0.0;
     for (long long i = (long long)blockIdx.x * kDotThreads + threadIdx.x; i < N; i += (long long)gridDim.x * kDotThreads) {
         x[i] = fma(a, p[i], x[i]);
@@ -138,16 +139,20 @@ __global__ void __launch_bounds__(kDotThreads) cg_update_xr_kernel(long long N, 
     }
 }
 
+// `it` is the iteration index of this call (a kernel argument).  rho and the frozen flag are double-buffered by its
+// parity: iteration it reads slot it & 1 and block 0 writes slot (it + 1) & 1, so no kernel reads a scalar that another
+// block of the same launch writes, and no separate "advance" launch is needed.
 __global__ void __launch_bounds__(kDotThreads) cg_update_p_kernel(long long N, const double* z, double* p,
                                                                    const double* __restrict__ dotp, CgScalars* sc,
-                                                                   double* __restrict__ hist, double* __restrict__ ab) {
+                                                                   double* __restrict__ hist, double* __restrict__ ab,
+                                                                   int it) {
     __shared__ double sh[kDotThreads];
-    const int it = sc->it;                               // advanced by cg_advance_kernel, a launch of its own
     double* hist_slot = hist ? hist + it + 1 : nullptr;
     double* ab_slot = ab ? ab + 2 * it : nullptr;
-    if (sc->done) {   // frozen: carry rho forward so that the parity bookkeeping stays valid
+    if (sc->done[it & 1]) {   // frozen: carry rho and the flag forward so that the parity bookkeeping stays valid
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             sc->rho[(it + 1) & 1] = sc->rho[it & 1];
+            sc->done[(it + 1) & 1] = 1;
             if (hist_slot) *hist_slot = hist_slot[-1];
             if (ab_slot) { ab_slot[0] = 0.0; ab_slot[1] = 0.0; }
         }
@@ -165,15 +170,8 @@ __global__ void __launch_bounds__(kDotThreads) cg_update_p_kernel(long long N, c
         if (hist_slot) *hist_slot = sqrt(rr);
         if (ab_slot) { ab_slot[0] = sc->a; ab_slot[1] = b; }
         sc->iters_done = it + 1;
+        sc->done[(it + 1) & 1] = (sc->tol2 > 0.0 && rr <= sc->tol2) ? 1 : 0;
     }
-}
-
-// The iteration counter may advance and `done` may be raised only after every block of update_p has read them:
-// separate 1-thread kernel.  Kernel arguments never depend on the iteration, so one captured CUDA graph of an
-// iteration can be replayed (grav_api.cu).
-__global__ void cg_advance_kernel(CgScalars* sc) {
-    sc->it += 1;
-    if (!sc->done && sc->tol2 > 0.0 && sc->rr <= sc->tol2) sc->done = 1;
 }
 
 cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, const double* minv, double lam, double* x, double* r,
@@ -191,25 +189,24 @@ cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc
 }
 
 cudaError_t launch_dot_pq(grav_ctx* c, const double* p, double lam, double* q, double* dotp, const CgScalars* sc,
-                          cudaStream_t s) {
-    dot_pq_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, p, lam, q, dotp, &sc->done);
+                          int it, cudaStream_t s) {
+    dot_pq_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, p, lam, q, dotp, &sc->done[it & 1]);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,
                                 const double* minv, double lam, double* z, const double* dotp_in, double* dotp_out,
-                                CgScalars* sc, cudaStream_t s) {
-    cg_update_xr_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, x, r, p, q, minv, lam, z, dotp_in, dotp_out, sc);
+                                CgScalars* sc, int it, cudaStream_t s) {
+    cg_update_xr_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, x, r, p, q, minv, lam, z, dotp_in, dotp_out, sc, it);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_cg_update_p(grav_ctx* c, const double* z, double* p, const double* dotp, CgScalars* sc, double* hist,
-                               double* ab, cudaStream_t s) {
-    cg_update_p_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, z, p, dotp, sc, hist, ab);
-    cg_advance_kernel<<<1, 1, 0, s>>>(sc);
-    c->launches += 2;
+                               double* ab, int it, cudaStream_t s) {
+    cg_update_p_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, z, p, dotp, sc, hist, ab, it);
+    c->launches++;
     return cudaGetLastError();
 }
 

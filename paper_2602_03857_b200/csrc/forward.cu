@@ -75,90 +75,131 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
+// work != NULL: persistent launch for small problems - a block copies the Psi tables (up to 140 KB) ONCE and then draws
+// (station tile, column chunk) items from the counter *work until none is left, instead of one block per item; which
+// block computes an item does not change what is written, so the result stays deterministic.
 template <int TPB, int UNROLL, int MINB, bool LOG2D>
 __global__ void __launch_bounds__(TPB, MINB) forward_nodes_staged_kernel(Geom g, PsiDev pd,
                                                                          const double2* __restrict__ cnode,
                                                                          double* __restrict__ partial,
                                                                          int cols_per_chunk,
-                                                                         const int* __restrict__ done) {
+                                                                         const int* __restrict__ done,
+                                                                         int* __restrict__ work, int ntiles,
+                                                                         int nitems) {
     extern __shared__ double2 s_tab[];
+    __shared__ int s_item;
     if (done && *done) return;
     const PsiTabView tb = psi_tables_load<LOG2D>(s_tab, pd);
     double2* s_stage = s_tab + (LOG2D ? psi_log2d_smem_entries(pd) : (size_t)kTabEntries * kRep);
-    const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
-    const long long il = i < g.N ? i : g.N - 1;
-    const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
-    const int col0 = blockIdx.y * cols_per_chunk;
-    const int col1 = min(col0 + cols_per_chunk, g.ncol);
     const int cpt = kFwdStage / g.nzp;                       // whole columns per tile (>= 1, checked by the launcher)
-    const int ntile = (col1 - col0 + cpt - 1) / cpt;
-    auto prefetch = [&](int t) {
-        const int c0 = col0 + t * cpt;
-        const int nn = (min(c0 + cpt, col1) - c0) * g.nzp;
-        const double2* src = cnode + (long long)c0 * g.nzp;
-        double2* dst = s_stage + (t & 1) * kFwdStage;
-        for (int e = threadIdx.x; e < nn; e += TPB) cp_async16(dst + e, src + e);
-        cp_async_commit();
-    };
-    double acc = 0.0;
-    int a = col0 / g.nyp, b = col0 - a * g.nyp;
-    double X = __ldg(g.xn + a) - xo;
-    if (ntile > 0) prefetch(0);
-    for (int t = 0; t < ntile; ++t) {
-        if (t + 1 < ntile) { prefetch(t + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
-        __syncthreads();
-        const int tc0 = col0 + t * cpt;
-        const int tc1 = min(tc0 + cpt, col1);
-        const double2* sc = s_stage + (t & 1) * kFwdStage;
-        for (int col = tc0; col < tc1; ++col, sc += g.nzp) {
-            const double Y = __ldg(g.yn + b) - yo;
-            const PsiColumn pc = psi_column(X, Y);
-            double colacc = 0.0;
-#pragma unroll UNROLL
-            for (int c = 0; c < g.nzp; ++c) {
-                const double2 cz = sc[c];
-                colacc = fma(cz.x, psi_eval<LOG2D>(tb, pc, cz.y - zo), colacc);
-            }
-            acc = fma(colacc, pc.s, acc);
-            if (++b == g.nyp) {
-                b = 0;
-                ++a;
-                if (a < g.nxp) X = __ldg(g.xn + a) - xo;
-            }
+    for (;;) {
+        int bx = blockIdx.x, by = blockIdx.y;
+        if (work) {
+            __syncthreads();                                 // the previous item's s_item and stage buffers are done with
+            if (threadIdx.x == 0) s_item = atomicAdd(work, 1);
+            __syncthreads();
+            const int item = s_item;
+            if (item >= nitems) break;
+            by = item / ntiles;                              // tile index fastest: neighbours in time share a chunk's stream
+            bx = item - by * ntiles;
         }
-        __syncthreads();      // everyone is done with buffer t&1 before tile t+2 is copied into it
+        const long long i = (long long)bx * TPB + threadIdx.x;
+        const long long il = i < g.N ? i : g.N - 1;
+        const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
+        const int col0 = by * cols_per_chunk;
+        const int col1 = min(col0 + cols_per_chunk, g.ncol);
+        const int ntile = (col1 - col0 + cpt - 1) / cpt;
+        auto prefetch = [&](int t) {
+            const int c0 = col0 + t * cpt;
+            const int nn = (min(c0 + cpt, col1) - c0) * g.nzp;
+            const double2* src = cnode + (long long)c0 * g.nzp;
+            double2* dst = s_stage + (t & 1) * kFwdStage;
+            for (int e = threadIdx.x; e < nn; e += TPB) cp_async16(dst + e, src + e);
+            cp_async_commit();
+        };
+        double acc = 0.0;
+        int a = col0 / g.nyp, b = col0 - a * g.nyp;
+        double X = __ldg(g.xn + a) - xo;
+        if (ntile > 0) prefetch(0);
+        for (int t = 0; t < ntile; ++t) {
+            if (t + 1 < ntile) { prefetch(t + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+            __syncthreads();
+            const int tc0 = col0 + t * cpt;
+            const int tc1 = min(tc0 + cpt, col1);
+            const double2* sc = s_stage + (t & 1) * kFwdStage;
+            for (int col = tc0; col < tc1; ++col, sc += g.nzp) {
+                const double Y = __ldg(g.yn + b) - yo;
+                const PsiColumn pc = psi_column(X, Y);
+                double colacc = 0.0;
+                // UNROLL independent evaluations in flight; the column's remainder in groups of 4 and then singly (a
+                // plain `#pragma unroll UNROLL` leaves up to UNROLL - 1 nodes per column - 9 of 33 at config 2 - to a
+                // one-at-a-time loop)
+                int c = 0;
+                for (; c + UNROLL <= g.nzp; c += UNROLL) {
+#pragma unroll
+                    for (int u = 0; u < UNROLL; ++u) {
+                        const double2 cz = sc[c + u];
+                        colacc = fma(cz.x, psi_eval<LOG2D>(tb, pc, cz.y - zo), colacc);
+                    }
+                }
+                for (; c + 4 <= g.nzp; c += 4) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const double2 cz = sc[c + u];
+                        colacc = fma(cz.x, psi_eval<LOG2D>(tb, pc, cz.y - zo), colacc);
+                    }
+                }
+#pragma unroll 1
+                for (; c < g.nzp; ++c) {
+                    const double2 cz = sc[c];
+                    colacc = fma(cz.x, psi_eval<LOG2D>(tb, pc, cz.y - zo), colacc);
+                }
+                acc = fma(colacc, pc.s, acc);
+                if (++b == g.nyp) {
+                    b = 0;
+                    ++a;
+                    if (a < g.nxp) X = __ldg(g.xn + a) - xo;
+                }
+            }
+            __syncthreads();      // everyone is done with buffer t&1 before tile t+2 is copied into it
+        }
+        if (i < g.N) partial[(long long)by * g.N + i] = acc;
+        if (!work) break;
     }
-    if (i < g.N) partial[(long long)blockIdx.y * g.N + i] = acc;
 }
 
 // d = scale * sum_chunks partial (+ lam * p).  With dotp != NULL also writes kDotBlocks block partials of p . d (CG:
 // delta).  A block is kRedX stations x kRedY chunk lanes: lane y adds chunks y, y + kRedY, ... in increasing order and
 // the kRedY lane sums are added in a fixed tree, so the result does not depend on the launch; blocks stride over the
 // station tiles.
-constexpr int kRedX = 32, kRedY = kDotThreads / kRedX;
-
+// RX = 32 stations per block (8 chunk lanes) for the large problems, 8 stations x 32 lanes where the stations are few and
+// the chunks many (config 1: 256 stations, 289 one-column chunks) - a property of the context, fixed at its creation.
+template <int RX>
 __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N, int nchunk,
                                                                       const double* __restrict__ partial, double scale,
                                                                       double lam, const double* __restrict__ p,
                                                                       double* __restrict__ d, double* __restrict__ dotp,
                                                                       const int* __restrict__ done) {
+    constexpr int RY = kDotThreads / RX;
     if (done && *done) {      // frozen CG: keep the exchanged partials finite
         if (dotp && threadIdx.x == 0) dotp[blockIdx.x] = 0.0;
         return;
     }
-    __shared__ double sh[kRedY][kRedX + 1];
-    __shared__ double shd[kRedX];
-    const int tx = threadIdx.x & (kRedX - 1), ty = threadIdx.x / kRedX;
+    __shared__ double sh[RY][RX + 1];
+    __shared__ double shd[RX];
+    const int tx = threadIdx.x & (RX - 1), ty = threadIdx.x / RX;
     double loc = 0.0;        // dot partial of the stations this thread finishes (ty == 0 only)
-    for (long long i0 = (long long)blockIdx.x * kRedX; i0 < N; i0 += (long long)gridDim.x * kRedX) {
+    for (long long i0 = (long long)blockIdx.x * RX; i0 < N; i0 += (long long)gridDim.x * RX) {
         const long long i = i0 + tx;
         double s = 0.0;
-        if (i < N)
-            for (int ch = ty; ch < nchunk; ch += kRedY) s += partial[(long long)ch * N + i];
+        if (i < N) {
+#pragma unroll 4
+            for (int ch = ty; ch < nchunk; ch += RY) s += partial[(long long)ch * N + i];
+        }
         sh[ty][tx] = s;
         __syncthreads();
 #pragma unroll
-        for (int h = kRedY / 2; h > 0; h >>= 1) {
+        for (int h = RY / 2; h > 0; h >>= 1) {
             if (ty < h) sh[ty][tx] += sh[ty + h][tx];
             __syncthreads();
         }
@@ -179,7 +220,7 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
         if (threadIdx.x == 0) {
             double t = 0.0;
 #pragma unroll
-            for (int k = 0; k < kRedX; ++k) t += shd[k];
+            for (int k = 0; k < RX; ++k) t += shd[k];
             dotp[blockIdx.x] = t;
         }
     }
@@ -201,7 +242,7 @@ static cudaError_t fwd_launch_unstaged(grav_ctx* c, const double2* cnode, double
 }
 
 template <int TPB, int UNROLL, int MINB, bool LOG2D>
-static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done,
+static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done, int* work,
                                      cudaStream_t s) {
     if (c->g.nzp > kFwdStage) return fwd_launch_unstaged<256, 8, 2, false>(c, cnode, partial, done, s);
     constexpr size_t stage = 2 * kFwdStage * sizeof(double2);
@@ -213,27 +254,42 @@ static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* 
                                             psi_smem_max<LOG2D>() + stage, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
-    dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), c->plan.fwd_nchunk);
+    const int ntiles = (int)((c->g.N + TPB - 1) / TPB);
+    const long long nitems = (long long)ntiles * c->plan.fwd_nchunk;
+    dim3 grid((unsigned)ntiles, c->plan.fwd_nchunk);
+    if (c->plan.persistent && nitems < (1ll << 31)) {
+        cudaError_t e = cudaMemsetAsync(work, 0, sizeof(int), s);
+        if (e != cudaSuccess) return e;
+        const long long resident = (long long)c->plan.sms * MINB;
+        grid = dim3((unsigned)(nitems < resident ? nitems : resident), 1);
+    } else {
+        work = nullptr;
+    }
     forward_nodes_staged_kernel<TPB, UNROLL, MINB, LOG2D><<<grid, TPB, smem, s>>>(c->g, c->pd, cnode, partial,
-                                                                                  c->plan.fwd_cols_per_chunk, done);
+                                                                                  c->plan.fwd_cols_per_chunk, done,
+                                                                                  work, ntiles, (int)nitems);
     return cudaGetLastError();
 }
 
-cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* partial, const int* done, cudaStream_t s) {
+cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* partial, const int* done, int* work,
+                                 cudaStream_t s) {
     const double2* cnode = reinterpret_cast<const double2*>(cnode_);
     cudaError_t e;
     if (c->psi_variant == 1) e = fwd_launch_unstaged<128, 1, 4, true>(c, cnode, partial, done, s);
-    else if (use_log2d(c)) e = fwd_launch_staged<512, 12, 1, true>(c, cnode, partial, done, s);
-    else e = fwd_launch_staged<256, 8, 2, false>(c, cnode, partial, done, s);
+    else if (use_log2d(c)) e = fwd_launch_staged<512, 12, 1, true>(c, cnode, partial, done, work, s);
+    else e = fwd_launch_staged<256, 8, 2, false>(c, cnode, partial, done, work, s);
     c->launches++;
     return e;
 }
 
 cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double scale, double lam, const double* p,
-                                  double* d, double* dot_partial, const CgScalars* sc, cudaStream_t s) {
-    const int* done = sc ? &sc->done : nullptr;
-    forward_reduce_kernel<<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, c->plan.fwd_nchunk, partial, scale, lam, p, d,
-                                                             dot_partial, done);
+                                  double* d, double* dot_partial, const int* done, cudaStream_t s) {
+    if (c->plan.fwd_reduce_rx == 8)
+        forward_reduce_kernel<8><<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, c->plan.fwd_nchunk, partial, scale, lam, p, d,
+                                                                    dot_partial, done);
+    else
+        forward_reduce_kernel<32><<<kDotBlocks, kDotThreads, 0, s>>>(c->g.N, c->plan.fwd_nchunk, partial, scale, lam, p,
+                                                                     d, dot_partial, done);
     c->launches++;
     return cudaGetLastError();
 }

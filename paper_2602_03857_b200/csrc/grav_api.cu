@@ -36,8 +36,13 @@ int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Launch plan: enough blocks to fill 148 SMs several times over, fixed per context => deterministic sums.
 // log2d: the context's geometry admits the 2-D log table (psi.cuh LOG2D): kernels of 512 / 256 threads, 1 block per SM.
-void make_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
+void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     p.log2d = log2d ? 1 : 0;
+    p.sms = sms > 0 ? sms : 148;
+    // Small problems (configs 1-2) run the node kernels persistently: with ~50 waves of short blocks the per-block table
+    // fill (up to 140 KB from L2) and pipeline start cost 15-20 % of a launch there; from ~1e10 evaluations per product the
+    // plain grid is as fast or faster (profiles/r2_small_configs.md).
+    p.persistent = (log2d && (double)g.N * (double)g.Nn < 1e10) ? 1 : 0;
     // Blocks of one launch all take the same time, so a grid of W.f waves of resident blocks costs ceil(W.f) waves:
     // with ~5 waves (the first plan) up to 18 % of the launch was tail.  ~100 blocks per SM keeps the tail <= 2-3 %
     // (profiles/r1_tail_and_variants.md); the price is a larger partial buffer (<= 64 MB), read once.
@@ -52,6 +57,7 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     if (want < 1) want = 1;
     p.fwd_cols_per_chunk = ceil_div(g.ncol, want);
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
+    p.fwd_reduce_rx = g.N < 32 * kDotBlocks ? 8 : 32;      // few stations: 8 per block and 32 chunk lanes (forward.cu)
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
     // KC nodes per thread: the per-(thread, station) set-up is shared by KC evaluations but the column is padded to a
     // multiple of KC.  With the 2-D log table the compiled (threads, KC) variants measure 114.3 (256, 8), 112.5 (384, 6),
@@ -81,6 +87,7 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     // than SMs, go down to 16 stations per chunk
     int maxchunk = ceil_div(g.N, 64);
     if ((long long)maxchunk * p.adj_blocks < 148) maxchunk = ceil_div(g.N, 16);
+    if ((long long)maxchunk * p.adj_blocks < 148) maxchunk = ceil_div(g.N, 8);
     if (want > maxchunk) want = maxchunk;
     if (want > 256) want = 256;
     if (want < 1) want = 1;
@@ -109,6 +116,7 @@ void make_layout(const Geom& g, const Plan& p, int world, WsLayout& L) {
     L.stage_m = take(g.M * D);
     L.stage_n = take(g.N * D);
     L.stage_hist = take(4096 * D);
+    L.work = take(64);                         // item counters of persistent launches (forward, adjoint)
     L.inv_dm = take(g.M * D);
     L.inv_r = take(g.N * D);
     L.inv_dd = take(g.N * D);
@@ -154,9 +162,9 @@ grav_status adjoint_to_tnode(grav_ctx* c, const double* v, const int* done, cuda
     double* part = wsp<double>(c, c->lay.adj_partial);
     double* tn = wsp<double>(c, c->lay.tnode);
     if (c->plan.adj_nchunk == 1) {
-        CK(launch_adjoint_nodes(c, v, tn, done, s), "adjoint_nodes");
+        CK(launch_adjoint_nodes(c, v, tn, done, wsp<int>(c, c->lay.work) + 1, s), "adjoint_nodes");
     } else {
-        CK(launch_adjoint_nodes(c, v, part, done, s), "adjoint_nodes");
+        CK(launch_adjoint_nodes(c, v, part, done, wsp<int>(c, c->lay.work) + 1, s), "adjoint_nodes");
         CK(launch_adjoint_reduce(c, part, c->plan.adj_nchunk, tn, s), "adjoint_reduce");
     }
     if (c->comm.world > 1) {
@@ -280,7 +288,9 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
     c->comm.world = 1;
     // tiny problems (config 1) would pay more for filling ~100 KB of table per block than they gain: the table is
     // built whenever the geometry admits it, but it is the default only from 5e7 evaluations per product
-    make_plan(g, c->pd, c->pd.tab2d != nullptr && (double)g.N * (double)g.Nn >= 5e7, c->plan);
+    int sms = 148;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) sms = 148;
+    make_plan(g, c->pd, c->pd.tab2d != nullptr && (double)g.N * (double)g.Nn >= 5e7, sms, c->plan);
     make_layout(g, c->plan, 1, c->lay);
     *out = c;
     return GRAV_OK;
@@ -382,7 +392,7 @@ grav_status grav_forward(grav_ctx* c, const double* u, double* d, void* stream) 
     double* cn = wsp<double>(c, c->lay.cnode);
     double* part = wsp<double>(c, c->lay.fwd_partial);
     CK(launch_cell_to_node(c, u, nullptr, cn, s), "cell_to_node");
-    CK(launch_forward_nodes(c, cn, part, nullptr, s), "forward_nodes");
+    CK(launch_forward_nodes(c, cn, part, nullptr, wsp<int>(c, c->lay.work), s), "forward_nodes");
     CK(launch_forward_reduce(c, part, c->g.gamma, 0.0, nullptr, d, nullptr, nullptr, s), "forward_reduce");
     return GRAV_OK;
 }
@@ -501,24 +511,25 @@ grav_status grav_dataspace_cg(grav_ctx* c, const double* dobs, const double* w, 
     if ((st = exchange(c, dotA, 3 * kDotBlocks, s))) return st;
     CK(launch_cg_init_finish(c, dotA, sc, rtol, resume, state ? state->rho_dev : nullptr, hist, s), "cg_init_finish");
     for (int it = 0; it < iters; ++it) {
+        const int* done = &sc->done[it & 1];
         if (mode == GRAV_MATRIX_FREE) {
             // q = gamma^2 * Fwd( S^T W^-2 S Adj(p) ) + lambda p
-            st = adjoint_to_tnode(c, p, &sc->done, s);
+            st = adjoint_to_tnode(c, p, done, s);
             if (st) return st;
             CK(launch_node_to_cell(c, tnode, w, g.gamma, gcell, s), "node_to_cell");
             CK(launch_cell_to_node(c, gcell, nullptr, cnode, s), "cell_to_node");
-            CK(launch_forward_nodes(c, cnode, fpart, &sc->done, s), "forward_nodes");
-            CK(launch_forward_reduce(c, fpart, g.gamma, lambda, p, q, dotA, sc, s), "forward_reduce");
+            CK(launch_forward_nodes(c, cnode, fpart, done, wsp<int>(c, c->lay.work), s), "forward_nodes");
+            CK(launch_forward_reduce(c, fpart, g.gamma, lambda, p, q, dotA, done, s), "forward_reduce");
         } else {
             CK(launch_gemvt(c, G, c->stored_elem, p, w, gcell, wsp<double>(c, c->lay.gemvt_partial), s), "gemvt");
             if ((st = exchange(c, gcell, g.M, s))) return st;
             CK(launch_gemv(c, G, c->stored_elem, gcell, q, s), "gemv");
-            CK(launch_dot_pq(c, p, lambda, q, dotA, sc, s), "dot_pq");
+            CK(launch_dot_pq(c, p, lambda, q, dotA, sc, it, s), "dot_pq");
         }
         if ((st = exchange(c, dotA, kDotBlocks, s))) return st;
-        CK(launch_cg_update_xr(c, x, r, p, q, precond, lambda, z, dotA, dotB, sc, s), "cg_update_xr");
+        CK(launch_cg_update_xr(c, x, r, p, q, precond, lambda, z, dotA, dotB, sc, it, s), "cg_update_xr");
         if ((st = exchange(c, dotB, 2 * kDotBlocks, s))) return st;
-        CK(launch_cg_update_p(c, z, p, dotB, sc, hist, ab, s), "cg_update_p");
+        CK(launch_cg_update_p(c, z, p, dotB, sc, hist, ab, it, s), "cg_update_p");
     }
     if (alpha != x) CK(cudaMemcpyAsync(alpha, x, g.N * sizeof(double), cudaMemcpyDeviceToDevice, s), "copy alpha");
     if (state) CK(cudaMemcpyAsync(state->rho_dev, &sc->rho[iters & 1], sizeof(double), cudaMemcpyDeviceToDevice, s), "copy rho");

@@ -29,6 +29,9 @@ struct Geom {
 struct Plan {
     // forward: grid (obs tiles, node-column chunks)
     int log2d;             // 1: kernels use the 2-D log table (psi.cuh LOG2D)
+    int persistent;        // 1: node kernels launch one block per SM slot that draws work items from a counter
+    int sms;               // multiprocessors of the device
+    int fwd_reduce_rx;     // stations per block of forward_reduce (32, or 8 when stations are few and chunks many)
     int fwd_tpb, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
     // adjoint: grid (node-thread blocks, station chunks)
     int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;
@@ -44,12 +47,12 @@ constexpr int kDotThreads = 256;
 struct CgScalars {
     double rho[2];
     double delta, a, b, dnorm2, tol2, rr;     // rr = ||r||^2 of the last finished iteration
-    int done, iters_done, it;                 // it: iteration counter of the current call (cg_advance_kernel)
+    int done[2], iters_done;                  // done: frozen flag (rtol reached), by iteration parity like rho
 };
 
 struct WsLayout {
     size_t cnode, tnode, fwd_partial, adj_partial, gcell, cg_x, cg_r, cg_p, cg_q, cg_z, cg_w, dot_partial, scalars,
-        stage_m, stage_n, stage_hist, inv_dm, inv_r, inv_dd, inv_try, inv_scal, gram_partial, comm_gather, matfree_end,
+        stage_m, stage_n, stage_hist, work, inv_dm, inv_r, inv_dd, inv_try, inv_scal, gram_partial, comm_gather, matfree_end,
         gemvt_partial, gstore;
 };
 
@@ -105,12 +108,15 @@ cudaError_t launch_node_to_cell(grav_ctx* c, const double* tnode, const double* 
                                 cudaStream_t s);
 cudaError_t launch_depth_weights(grav_ctx* c, double beta, double z0, double* w, cudaStream_t s);
 // --- forward.cu : partial sums of sum_n cnode[n] Psi(node_n - obs_i) into fwd_partial
-cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, cudaStream_t s);
+// work: one int of device scratch (the item counter of a persistent launch, plan.persistent)
+cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode, double* partial, const int* done, int* work,
+                                 cudaStream_t s);
 // d = scale * sum_chunks partial (+ lam * p if p != NULL); if dot_partial != NULL also block partials of p.d
 cudaError_t launch_forward_reduce(grav_ctx* c, const double* partial, double scale, double lam, const double* p,
-                                  double* d, double* dot_partial, const CgScalars* sc, cudaStream_t s);
+                                  double* d, double* dot_partial, const int* done, cudaStream_t s);
 // --- adjoint.cu : tnode[n] = sum_i v_i Psi(node_n - obs_i)
-cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, cudaStream_t s);
+cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, const int* done, int* work,
+                                 cudaStream_t s);
 cudaError_t launch_adjoint_reduce(grav_ctx* c, const double* partial, int nchunk, double* tnode, cudaStream_t s);
 // --- cg.cu
 cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, const double* minv, double lam, double* x, double* r,
@@ -118,12 +124,12 @@ cudaError_t launch_cg_init(grav_ctx* c, const double* dobs, const double* minv, 
 cudaError_t launch_cg_init_finish(grav_ctx* c, const double* dotp, CgScalars* sc, double rtol, int resume,
                                   const double* rho_in, double* hist, cudaStream_t s);
 cudaError_t launch_dot_pq(grav_ctx* c, const double* p, double lam, double* q, double* dotp, const CgScalars* sc,
-                          cudaStream_t s);
+                          int it, cudaStream_t s);
 cudaError_t launch_cg_update_xr(grav_ctx* c, double* x, double* r, const double* p, const double* q,
                                 const double* minv, double lam, double* z, const double* dotp_in, double* dotp_out,
-                                CgScalars* sc, cudaStream_t s);
+                                CgScalars* sc, int it, cudaStream_t s);
 cudaError_t launch_cg_update_p(grav_ctx* c, const double* z, double* p, const double* dotp, CgScalars* sc, double* hist,
-                               double* ab, cudaStream_t s);
+                               double* ab, int it, cudaStream_t s);
 // --- stored.cu
 cudaError_t launch_tabulate(grav_ctx* c, void* G, int elem, cudaStream_t s);
 cudaError_t launch_gemv(grav_ctx* c, const void* G, int elem, const double* u, double* d, cudaStream_t s);
