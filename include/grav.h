@@ -182,6 +182,17 @@ typedef struct {
 } grav_comm;
 grav_status grav_set_comm(grav_ctx* ctx, const grav_comm* comm);
 
+/* Precision of the matrix-free evaluation ("using Float32 precision").
+ * GRAV_PREC_F64 (default): everything in FP64 (BJ).  GRAV_PREC_F32: grav_forward, grav_adjoint and the GRAV_MATRIX_FREE
+ * products inside grav_dataspace_cg / grav_invert evaluate Psi in Float32 - from coordinate differences formed in FP64,
+ * with the cancellation-free form of R + Y for Y < 0 - and accumulate in FP64; vectors stay FP64.  The per-pair family
+ * (grav_store_g, grav_gram_diag) always evaluates in FP64.  The Float32 closed form has a cancellation floor of
+ * ~(|X| + |Y| + |Z|) 2^-24 per corner term (~1e-3 m at 10 km, where far-field coefficients are 1e-5..1e-3 m): this mode
+ * reproduces the paper's precision for comparison, its error is reported by bench.py and it is NOT held to the 1e-10
+ * operator tolerance.  Errors: GRAV_EINVAL. */
+enum { GRAV_PREC_F64 = 0, GRAV_PREC_F32 = 1 };
+grav_status grav_set_precision(grav_ctx* ctx, int precision);
+
 /* Launch accounting: number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 long long grav_launch_count(const grav_ctx* ctx);
 /* FP64 DFMA-only microbenchmark: runs `iters` dependent-chain-free DFMA per thread on the whole device and
@@ -192,6 +203,14 @@ grav_status grav_fp64_peak_probe(int device, int iters, double* ninstr, double* 
  * sqrt / reciprocal; csrc/psi.cuh); variant 1: the same tilings with CUDA libm (sqrt, /, atan, log).  Both are tested
  * against the oracle; variant 1 exists for cross-checks and A/B timing. */
 grav_status grav_debug_set_psi_variant(grav_ctx* ctx, int variant);
+/* One Psi evaluation per argument triple with a device evaluator (tests compare them with the oracle's Psi argument by
+ * argument): variant 0 = hand-built FP64 evaluator with the 256-entry log table, 1 = CUDA libm FP64, 2 = Float32
+ * evaluator, 3 = hand-built FP64 evaluator with the exponent-and-mantissa log table (GRAV_ESTATE when the context has
+ * none; arguments of the logarithms must then lie in its range).  X_dev, Y_dev, Z_dev, out_dev: n doubles each.
+ * Variants 0, 2, 3 return Psi + (X + Y) k0 ln 2 with k0 = grav_debug_k0(ctx) (clamped to +-100 for variant 2): the
+ * offset that cancels exactly in every signed sum of the library.  Needs no workspace. */
+grav_status grav_debug_psi_eval_device(grav_ctx* ctx, int variant, long long n, const double* X_dev, const double* Y_dev,
+                                       const double* Z_dev, double* out_dev, void* stream);
 /* Which log table the variant-0 kernels use: -1 the context's default (grav_debug_log2d_default), 0 the 256-entry
  * table with explicit exponent handling, 1 the exponent-and-mantissa table (GRAV_ESTATE when the geometry does not
  * admit it).  Both form the same sums in the same order; they differ by rounding only.  For tests and A/B timing. */

@@ -15,6 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libgrav.so")
 
 MATRIX_FREE, STORED_F64, STORED_F32 = 0, 1, 2
+PREC_F64, PREC_F32 = 0, 1
 
 EXPORTS = [
     "grav_mesh_create", "grav_mesh_destroy", "grav_sizes", "grav_workspace_bytes", "grav_set_workspace",
@@ -23,6 +24,7 @@ EXPORTS = [
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
     "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_eval_host",
     "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_log2d_default", "grav_debug_set_log2d", "grav_set_comm",
+    "grav_set_precision", "grav_debug_psi_eval_device",
 ]
 
 # include/grav.h: grav_comm
@@ -103,6 +105,10 @@ def load():
     L.grav_debug_psi_eval_host.argtypes = [d, d, d, i, i]
     L.grav_debug_set_log2d.restype = i
     L.grav_debug_set_log2d.argtypes = [vp, i]
+    L.grav_set_precision.restype = i
+    L.grav_set_precision.argtypes = [vp, i]
+    L.grav_debug_psi_eval_device.restype = i
+    L.grav_debug_psi_eval_device.argtypes = [vp, i, ll, vp, vp, vp, vp, vp]
     L.grav_set_comm.restype = i
     L.grav_set_comm.argtypes = [vp, C.POINTER(_Comm)]
     L.grav_debug_k0.restype = i
@@ -350,6 +356,19 @@ class GravContext:
             _check(self._lib.grav_set_comm(self._h, C.byref(cs)))
         mode, self.ws, self.mode = self.mode, None, None
         self.set_mode(mode)
+
+    def set_precision(self, fp32):
+        """Matrix-free evaluation in Float32 (True; the paper's precision, FP64 accumulation) or FP64 (False, default)."""
+        _check(self._lib.grav_set_precision(self._h, PREC_F32 if fp32 else PREC_F64))
+
+    def psi_eval_device(self, variant, X, Y, Z):
+        """Psi (+ the k0 offset for variants 0, 2, 3) of the device evaluator `variant` at the argument triples given as
+        CUDA float64 tensors (include/grav.h: grav_debug_psi_eval_device)."""
+        n = X.numel()
+        out = self._new(n)
+        _check(self._lib.grav_debug_psi_eval_device(self._h, int(variant), n, _dev(X, n, "X"), _dev(Y, n, "Y"),
+                                                    _dev(Z, n, "Z"), _dev(out, n, "out"), _stream()))
+        return out
 
     def set_psi_variant(self, variant):
         """0: hand-built evaluator (default); 1: CUDA libm (cross-check)."""

@@ -21,7 +21,8 @@ namespace grav {
 
 constexpr int kAdjObsTile = 256;
 
-// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table
+// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table,
+// 3 = the Float32 evaluator psi_f32 with FP64 accumulation (grav_set_precision)
 // work != NULL: persistent launch for small problems (see forward.cu): the block fills the tables once and draws
 // (node-thread block, station chunk) items from the counter.
 template <int TPB, int KC, int MINB, int EV>
@@ -34,7 +35,8 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
     __shared__ int s_item;
     PsiTabView tb;
-    if (EV != 0) tb = psi_tables_load<EV == 2>(s_tab, pd);
+    if (EV == 1 || EV == 2) tb = psi_tables_load<EV == 2>(s_tab, pd);
+    const float inv_scale = psi_f32_inv_scale(pd.k0);
     const long long nthreads = (long long)g.ncol * ncg;
     for (;;) {
         int bx = blockIdx.x, by = blockIdx.y;
@@ -74,11 +76,16 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
             for (int j = 0; j < cnt; ++j) {
                 const double4 o = s_obs[j];
                 const double X = xa - o.x, Y = yb - o.y;
-                if (EV != 0) {
+                if (EV == 1 || EV == 2) {
                     const PsiColumn pc = psi_column(X, Y);
                     const double vs = o.w * pc.s;
 #pragma unroll
                     for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
+                } else if (EV == 3) {
+                    const float Xf = (float)X, Yf = (float)Y;
+#pragma unroll
+                    for (int k = 0; k < KC; ++k)
+                        acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale), acc[k]);
                 } else {
                     const double XY = X * Y;
                     const double Q = fma(Y, Y, X * X);
@@ -135,9 +142,9 @@ template <int TPB, int KC, int MINB, int EV>
 static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, const int* done, int* work,
                               cudaStream_t s) {
     // the opt-in is sized for the largest 2-D table, the launch for this context's table
-    const size_t smem = EV == 0 ? 0 : psi_smem_bytes<EV == 2>(c->pd);
+    const size_t smem = (EV == 1 || EV == 2) ? psi_smem_bytes<EV == 2>(c->pd) : 0;
     static unsigned long long smem_set = 0;
-    if (EV != 0) {
+    if (EV == 1 || EV == 2) {
         cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, psi_smem_max<EV == 2>(), c->device,
                                             &smem_set);
         if (e != cudaSuccess) return e;
@@ -147,7 +154,7 @@ static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, con
     const int nblocks = (int)((nthreads + TPB - 1) / TPB);
     const long long nitems = (long long)nblocks * c->plan.adj_nchunk;
     dim3 grid((unsigned)nblocks, c->plan.adj_nchunk);
-    if (c->plan.persistent && EV != 0 && nitems < (1ll << 31)) {
+    if (c->plan.persistent && (EV == 1 || EV == 2) && nitems < (1ll << 31)) {
         cudaError_t e = cudaMemsetAsync(work, 0, sizeof(int), s);
         if (e != cudaSuccess) return e;
         const long long resident = (long long)c->plan.sms * MINB;
@@ -166,6 +173,12 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
     const int kc = c->plan.adj_kc;           // the plan's choice of KC (grav_api.cu make_plan)
     cudaError_t e;
     if (c->psi_variant == 1) e = adj_launch<128, 4, 4, 0>(c, v, partial, done, work, s);
+    else if (c->psi_variant == 2) {      // Float32 evaluator: no tables, several blocks per SM
+        if (kc <= 4) e = adj_launch<256, 4, 4, 3>(c, v, partial, done, work, s);
+        else if (kc == 5) e = adj_launch<256, 5, 4, 3>(c, v, partial, done, work, s);
+        else if (kc == 6) e = adj_launch<256, 6, 4, 3>(c, v, partial, done, work, s);
+        else e = adj_launch<256, 8, 4, 3>(c, v, partial, done, work, s);
+    }
     else if (use_log2d(c)) {      // (threads, KC) pairs of make_plan's table
         if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, work, s);
         else if (kc == 5) e = adj_launch<384, 5, 1, 2>(c, v, partial, done, work, s);

@@ -12,21 +12,23 @@
 
 namespace grav {
 
-// Unstaged kernel: the (c_n, z_n) stream is read with LDG.  Used for the CUDA-libm cross-check (LIBM) and as the
-// fallback for node columns deeper than the stage buffer of the staged kernel below.
-template <int TPB, int UNROLL, int MINB, bool LIBM>
+// Unstaged kernel: the (c_n, z_n) stream is read with LDG.  EVAL 0: psi_eval with the 256-entry log table (fallback for
+// node columns deeper than the stage buffer of the staged kernel below); 1: CUDA libm in FP64 (cross-check); 2: the
+// Float32 evaluator psi_f32 with FP64 accumulation (grav_set_precision).
+template <int TPB, int UNROLL, int MINB, int EVAL>
 __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev pd, const double2* __restrict__ cnode,
                                                                   double* __restrict__ partial, int cols_per_chunk,
                                                                   const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
     PsiTabView tb;
-    if (!LIBM) tb = psi_tables_to_smem(s_tab, pd);
+    if (EVAL == 0) tb = psi_tables_to_smem(s_tab, pd);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
     const int col0 = blockIdx.y * cols_per_chunk;
     const int col1 = min(col0 + cols_per_chunk, g.ncol);
+    const float inv_scale = psi_f32_inv_scale(pd.k0);
     double acc = 0.0;
     int a = col0 / g.nyp, b = col0 - a * g.nyp;
     double X = __ldg(g.xn + a) - xo;
@@ -34,7 +36,7 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
         const double Y = __ldg(g.yn + b) - yo;
         const double2* __restrict__ cc = cnode + (long long)col * g.nzp;   // (c_n, zn[c]) pairs: one LDG.128
         double colacc = 0.0;
-        if (!LIBM) {
+        if (EVAL == 0) {
             const PsiColumn pc = psi_column(X, Y);
 #pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
@@ -42,12 +44,19 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
                 colacc = fma(cz.x, psi_eval<false>(tb, pc, cz.y - zo), colacc);
             }
             colacc *= pc.s;
-        } else {
+        } else if (EVAL == 1) {
             const double XY = X * Y;
             const double Q = fma(Y, Y, X * X);
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = __ldg(cc + c);
                 colacc = fma(cz.x, psi_libm(X, Y, cz.y - zo, XY, Q), colacc);
+            }
+        } else {
+            const float Xf = (float)X, Yf = (float)Y;
+#pragma unroll UNROLL
+            for (int c = 0; c < g.nzp; ++c) {
+                const double2 cz = __ldg(cc + c);
+                colacc = fma(cz.x, (double)psi_f32(Xf, Yf, (float)(cz.y - zo), inv_scale), colacc);
             }
         }
         acc += colacc;
@@ -226,17 +235,17 @@ __global__ void __launch_bounds__(kDotThreads) forward_reduce_kernel(long long N
     }
 }
 
-template <int TPB, int UNROLL, int MINB, bool LIBM>
+template <int TPB, int UNROLL, int MINB, int EVAL>
 static cudaError_t fwd_launch_unstaged(grav_ctx* c, const double2* cnode, double* partial, const int* done,
                                        cudaStream_t s) {
-    constexpr size_t smem = LIBM ? 0 : kTabSmemBytes;
+    constexpr size_t smem = EVAL == 0 ? kTabSmemBytes : 0;
     static unsigned long long smem_set = 0;
     if (smem > 48 * 1024) {
-        cudaError_t e = ensure_dynamic_smem(forward_nodes_kernel<TPB, UNROLL, MINB, LIBM>, smem, c->device, &smem_set);
+        cudaError_t e = ensure_dynamic_smem(forward_nodes_kernel<TPB, UNROLL, MINB, EVAL>, smem, c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
     dim3 grid((unsigned)((c->g.N + TPB - 1) / TPB), c->plan.fwd_nchunk);
-    forward_nodes_kernel<TPB, UNROLL, MINB, LIBM><<<grid, TPB, smem, s>>>(c->g, c->pd, cnode, partial,
+    forward_nodes_kernel<TPB, UNROLL, MINB, EVAL><<<grid, TPB, smem, s>>>(c->g, c->pd, cnode, partial,
                                                                           c->plan.fwd_cols_per_chunk, done);
     return cudaGetLastError();
 }
@@ -244,7 +253,7 @@ static cudaError_t fwd_launch_unstaged(grav_ctx* c, const double2* cnode, double
 template <int TPB, int UNROLL, int MINB, bool LOG2D>
 static cudaError_t fwd_launch_staged(grav_ctx* c, const double2* cnode, double* partial, const int* done, int* work,
                                      cudaStream_t s) {
-    if (c->g.nzp > kFwdStage) return fwd_launch_unstaged<256, 8, 2, false>(c, cnode, partial, done, s);
+    if (c->g.nzp > kFwdStage) return fwd_launch_unstaged<256, 8, 2, 0>(c, cnode, partial, done, s);
     constexpr size_t stage = 2 * kFwdStage * sizeof(double2);
     // the opt-in is sized for the largest 2-D table, the launch for this context's table
     const size_t smem = psi_smem_bytes<LOG2D>(c->pd) + stage;
@@ -275,7 +284,8 @@ cudaError_t launch_forward_nodes(grav_ctx* c, const double* cnode_, double* part
                                  cudaStream_t s) {
     const double2* cnode = reinterpret_cast<const double2*>(cnode_);
     cudaError_t e;
-    if (c->psi_variant == 1) e = fwd_launch_unstaged<128, 1, 4, true>(c, cnode, partial, done, s);
+    if (c->psi_variant == 1) e = fwd_launch_unstaged<128, 1, 4, 1>(c, cnode, partial, done, s);
+    else if (c->psi_variant == 2) e = fwd_launch_unstaged<256, 8, 4, 2>(c, cnode, partial, done, s);
     else if (use_log2d(c)) e = fwd_launch_staged<512, 12, 1, true>(c, cnode, partial, done, work, s);
     else e = fwd_launch_staged<256, 8, 2, false>(c, cnode, partial, done, work, s);
     c->launches++;

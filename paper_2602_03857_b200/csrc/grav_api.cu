@@ -353,6 +353,22 @@ grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {
     return GRAV_OK;
 }
 
+grav_status grav_set_precision(grav_ctx* c, int precision) {
+    if (!c || (precision != GRAV_PREC_F64 && precision != GRAV_PREC_F32)) return fail(GRAV_EINVAL, "bad context / precision");
+    c->psi_variant = precision == GRAV_PREC_F32 ? 2 : 0;
+    return GRAV_OK;
+}
+
+grav_status grav_debug_psi_eval_device(grav_ctx* c, int variant, long long n, const double* X, const double* Y,
+                                       const double* Z, double* out, void* stream) {
+    if (!c || !X || !Y || !Z || !out || n <= 0) return fail(GRAV_EINVAL, "NULL argument / n <= 0");
+    if (variant < 0 || variant > 3) return fail(GRAV_EINVAL, "variant must be 0..3");
+    if (variant == 3 && !c->pd.tab2d) return fail(GRAV_ESTATE, "the geometry does not admit the 2-D log table");
+    DeviceGuard dg(c->device);
+    CK(launch_psi_check(c, variant, n, X, Y, Z, out, (cudaStream_t)stream), "psi_check");
+    return GRAV_OK;
+}
+
 grav_status grav_debug_set_log2d(grav_ctx* c, int mode) {
     if (!c || mode < -1 || mode > 1) return fail(GRAV_EINVAL, "bad context / mode");
     if (mode == 1 && !c->pd.tab2d) return fail(GRAV_ESTATE, "the geometry does not admit the 2-D log table");

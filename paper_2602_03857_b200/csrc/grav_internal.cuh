@@ -77,7 +77,7 @@ struct grav_ctx {
     size_t ws_bytes;
     int stored_elem;         // 0 none, 8 FP64, 4 FP32
     grav::PsiDev pd;         // Psi tables (inside geom_dev), constants and the global exponent offset k0
-    int psi_variant;         // 0 hand-built evaluator, 1 CUDA libm
+    int psi_variant;         // 0 hand-built FP64 evaluator, 1 CUDA libm FP64, 2 Float32 evaluator (grav_set_precision)
     int log2d_force;         // -1: the plan's choice; 0 / 1: force the 256-entry / the 2-D log table (diagnostic)
     grav_comm comm;          // observation-sharded operation (world == 1: single rank, no callbacks)
     long long launches;
@@ -143,6 +143,9 @@ cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, doubl
 int gemvt_chunks(long long N);
 void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p);
 size_t gram_partial_doubles(const Geom& g, const Plan& p);
+// --- psi_check.cu : one Psi evaluation per argument triple with the chosen device evaluator (diagnostic)
+cudaError_t launch_psi_check(grav_ctx* c, int variant, long long n, const double* X, const double* Y, const double* Z,
+                             double* out, cudaStream_t s);
 // --- invert.cu : vector kernels of the outer model-update loop
 cudaError_t launch_inv_residual(grav_ctx* c, const double* r, double s, const double* dd, double* out, double* partial,
                                 cudaStream_t st);
