@@ -105,6 +105,8 @@ def parse():
     ap.add_argument("--paper-shape-matrix-free", action="store_true",
                     help="also run the outer inversion loop matrix-free in FP64 on the paper's shape (~1 min)")
     ap.add_argument("--no-stored", action="store_true", help="skip the stored-G (HBM-bound GEMV) measurement")
+    ap.add_argument("--no-fp32", action="store_true", help="skip the Float32 matrix-free leg")
+    ap.add_argument("--no-precond", action="store_true", help="skip the plain-vs-Jacobi CG iteration count (config 2)")
     ap.add_argument("--stored-config", type=int, default=3, help="config whose G is tabulated for the stored-G leg")
     return ap.parse_args()
 
@@ -311,6 +313,75 @@ def paper_shape_leg(local, matrix_free=False):
     return res
 
 
+def fp32_leg(cfgs, local):
+    """SURVEY.md 8(f) item 2, second half: the matrix-free products with the Float32 evaluator (the paper's precision,
+    P:203; grav_set_precision) on BJ configs and on the paper's Table 1 shape: time per product and the error against the
+    FP64 path of the same library (itself within 1e-10 of the oracle), as a fraction of the output's global max."""
+    import torch
+    from paper_2602_03857_b200 import binding, workloads
+    dev = torch.device("cuda", local)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    out = {}
+    for cfg in cfgs:
+        wl = workloads.make(cfg)
+        ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+        u = torch.as_tensor(np.ascontiguousarray(wl.m_true)).to(dev)
+        d64 = ctx.forward(u)
+        v = d64 + wl.noise_frac * float(d64.abs().max()) * torch.as_tensor(wl.noise()).to(dev)
+        g64 = ctx.adjoint(v)
+        ctx.set_precision(True)
+
+        def timed(fn):
+            fn(); torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record(); r = fn(); b.record(); torch.cuda.synchronize()
+            return a.elapsed_time(b), r
+
+        t_f, d32 = timed(lambda: ctx.forward(u))
+        t_a, g32 = timed(lambda: ctx.adjoint(v))
+        out[wl.name] = {"ms_forward": t_f, "ms_adjoint": t_a,
+                        "pairs_per_s_forward": float(wl.N) * wl.M / (t_f * 1e-3),
+                        "pairs_per_s_adjoint": float(wl.N) * wl.M / (t_a * 1e-3),
+                        "err_of_max_forward": float((d32 - d64).abs().max() / d64.abs().max()),
+                        "err_of_max_adjoint": float((g32 - g64).abs().max() / g64.abs().max()),
+                        "inputs": "u = true model, v = noisy data"}
+        ctx.close()
+        del ctx
+        torch.cuda.empty_cache()
+    out["note"] = ("Float32 Psi (FP64 coordinate differences, cancellation-free R + Y, FP64 accumulation); error vs the "
+                   "FP64 path as a fraction of max|output|; not held to the 1e-10 operator tolerance")
+    return out
+
+
+def precond_leg(cfg, local, rtol=1e-8, cap=1500):
+    """Jacobi-preconditioned CG (M = diag(G W^-2 G^T) + lambda from grav_gram_diag) against plain
+    CG on the data-space system of `cfg`: iterations until the recursive residual meets rtol * ||d_obs||."""
+    import torch
+    from paper_2602_03857_b200 import binding, workloads
+    wl = workloads.make(cfg)
+    dev = torch.device("cuda", local)
+    ctx = binding.GravContext(wl.xn, wl.yn, wl.zn, wl.xo, wl.yo, wl.zo, wl.gamma, device=local)
+    w = ctx.depth_weights(wl.beta, wl.z0)
+    d_clean = ctx.forward(torch.as_tensor(np.ascontiguousarray(wl.m_true)).to(dev))
+    d_obs = d_clean + wl.noise_frac * float(d_clean.abs().max()) * torch.as_tensor(wl.noise()).to(dev)
+    diag = ctx.gram_diag(w)
+    lam = wl.lam_factor * float(diag.mean().item())
+    res = {"workload": wl.name, "rtol": rtol, "lambda": lam, "cap": cap}
+    for name, pc in (("plain", None), ("jacobi", diag)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        out = ctx.dataspace_cg(d_obs, w, lam, cap, rtol=rtol, precond=pc, want_m=False)
+        hist = out["hist"].cpu().numpy()
+        dt = time.perf_counter() - t0
+        below = np.nonzero(hist <= rtol * hist[0])[0]
+        res[name] = {"iterations": int(below[0]) if below.size else None, "final_rel_residual": float(hist[-1] / hist[0]),
+                     "seconds_for_cap_launches": dt}
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    return res
+
+
 # ---------------------------------------------------------------------------------------------------------------
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores.  One step = forward + adjoint restricted
@@ -364,6 +435,8 @@ def run_ours(args):
     from paper_2602_03857_b200 import dist as gdist
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")       # rank / transport lines on stderr (the JSON line is stdout)
     rank, world, local = gdist.init_from_env("nccl")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
@@ -529,6 +602,33 @@ def run_ours(args):
             paper = {"error": f"{type(ex).__name__}: {ex}"[:300]}
             torch.cuda.empty_cache()
 
+    fp32 = None
+    if rank == 0 and world == 1 and not args.no_fp32:
+        sh.close()
+        try:
+            fp32 = fp32_leg(sorted({3, args.config, 6}), local)
+        except Exception as ex:
+            fp32 = {"error": f"{type(ex).__name__}: {ex}"[:300]}
+            torch.cuda.empty_cache()
+
+    precond = None
+    if rank == 0 and world == 1 and not args.no_precond:
+        sh.close()
+        try:
+            precond = precond_leg(2, local)
+        except Exception as ex:
+            precond = {"error": f"{type(ex).__name__}: {ex}"[:300]}
+            torch.cuda.empty_cache()
+
+    # per-rank kernel times (multi-GPU: the driver reads the spread)
+    per_rank = None
+    if world > 1:
+        t = torch.tensor([t_fwd, t_adj], dtype=torch.float64, device=dev)
+        allt = [torch.empty_like(t) for _ in range(world)]
+        torch.distributed.all_gather(allt, t)
+        per_rank = [{"rank": r, "stations": gdist.shard_range(N, world, r)[1] - gdist.shard_range(N, world, r)[0],
+                     "ms_forward": float(a[0]), "ms_adjoint": float(a[1])} for r, a in enumerate(allt)]
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -538,12 +638,14 @@ def run_ours(args):
             "config": {"workload": wl.name, "prisms": M, "stations": N, "nodes": Nn,
                        "pairs_per_step": pairs_per_step,
                        "step": "one data-space CG iteration (G^T p, W^-2, G(.), fused vector ops)",
-                       "parallelism": f"stations sharded over {world} rank(s); all-reduce of node sums + dot partials",
+                       "parallelism": f"stations sharded over {world} rank(s); all-gather of the (hi, lo) node-sum "
+                                      f"planes + all-reduce of the dot partials",
                        "l2": "flushed between steps (256 MiB write)", "lambda": lam,
                        "lambda_note": "1e-2 * trace(G W^-2 G^T) / N from the full Gram diagonal (grav_gram_diag)",
                        "ms_gram_diag": ms_gram, "pairs_per_s_gram_diag": float(Nloc) * M / (ms_gram * 1e-3)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "stored_g": stored, "paper_shape": paper,
+            "stored_g": stored, "paper_shape": paper, "fp32_matrix_free": fp32, "jacobi_pcg": precond,
+            "per_rank": per_rank,
         }
         print(json.dumps(line))
     sh.close()
