@@ -34,8 +34,10 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     if (done && *done) return;
     __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
     __shared__ int s_item;
+    __shared__ float s_at[kAtanN32];
     PsiTabView tb;
     if (EV == 1 || EV == 2) tb = psi_tables_load<EV == 2>(s_tab, pd);
+    if (EV == 3) psi_f32_atan_table(s_at, pd);
     const float inv_scale = psi_f32_inv_scale(pd.k0);
     const long long nthreads = (long long)g.ncol * ncg;
     for (;;) {
@@ -85,7 +87,7 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
                     const float Xf = (float)X, Yf = (float)Y;
 #pragma unroll
                     for (int k = 0; k < KC; ++k)
-                        acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale), acc[k]);
+                        acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale, s_at), acc[k]);
                 } else {
                     const double XY = X * Y;
                     const double Q = fma(Y, Y, X * X);

@@ -20,9 +20,11 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
                                                                   double* __restrict__ partial, int cols_per_chunk,
                                                                   const int* __restrict__ done) {
     extern __shared__ double2 s_tab[];
+    __shared__ float s_at[kAtanN32];
     if (done && *done) return;
     PsiTabView tb;
     if (EVAL == 0) tb = psi_tables_to_smem(s_tab, pd);
+    if (EVAL == 2) psi_f32_atan_table(s_at, pd);
     const long long i = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long il = i < g.N ? i : g.N - 1;
     const double xo = g.xo[il], yo = g.yo[il], zo = g.zo[il];
@@ -56,7 +58,7 @@ __global__ void __launch_bounds__(TPB, MINB) forward_nodes_kernel(Geom g, PsiDev
 #pragma unroll UNROLL
             for (int c = 0; c < g.nzp; ++c) {
                 const double2 cz = __ldg(cc + c);
-                colacc = fma(cz.x, (double)psi_f32(Xf, Yf, (float)(cz.y - zo), inv_scale), colacc);
+                colacc = fma(cz.x, (double)psi_f32(Xf, Yf, (float)(cz.y - zo), inv_scale, s_at), colacc);
             }
         }
         acc += colacc;

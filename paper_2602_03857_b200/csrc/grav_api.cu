@@ -222,7 +222,7 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
 
     const size_t ntab = sizeof(PsiTablesHost) / sizeof(double);
     const size_t ntab2d = (size_t)kLog2dMaxBinades * 256 * 2;
-    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2d + 8 * 32;   // each array 256-byte aligned
+    const size_t nd = (size_t)g.nxp + g.nyp + g.nzp + 3 * (size_t)nobs + ntab + ntab2d + kAtanN32 + 9 * 32;   // each array 256-byte aligned
     std::vector<double> host;
     try { host.assign(nd, 0.0); } catch (...) { delete c; return fail(GRAV_ENOMEM, "host allocation failed"); }
     void* dev = nullptr;
@@ -251,6 +251,9 @@ grav_status grav_mesh_create(grav_ctx** out, int nx, int ny, int nz, const doubl
         psi_tables_generate(&tabs, c->pd.k0);
         c->pd.tab = reinterpret_cast<const double2*>(put(reinterpret_cast<const double*>(&tabs), ntab));
         c->pd.k = psi_consts_make(c->pd.k0);
+        double at32[kAtanN32];
+        psi_f32_atan_generate(at32);
+        c->pd.atan32 = put(at32, kAtanN32);
         // 2-D log table: arguments a = R + Y obey Zmin^2 / (2 Rmax) <= a <= 2 Rmax, with Zmin the smallest vertical
         // station-node distance and Rmax the largest station-node distance
         c->pd.tab2d = nullptr; c->pd.nb2d = 0; c->pd.emin2d_biased = 0;

@@ -15,6 +15,8 @@ __global__ void __launch_bounds__(256) psi_check_kernel(PsiDev pd, long long n, 
                                                          const double* __restrict__ Y, const double* __restrict__ Z,
                                                          double* __restrict__ out) {
     extern __shared__ double2 s_tab[];
+    __shared__ float s_at[kAtanN32];
+    if (VARIANT == 2) psi_f32_atan_table(s_at, pd);
     PsiTabView tb;
     if (VARIANT == 0) tb = psi_tables_to_smem(s_tab, pd);
     if (VARIANT == 3) tb = psi_tables_to_smem_2d(s_tab, pd);
@@ -22,7 +24,7 @@ __global__ void __launch_bounds__(256) psi_check_kernel(PsiDev pd, long long n, 
         const double x = X[i], y = Y[i], z = Z[i];
         double v;
         if (VARIANT == 1) v = psi_libm(x, y, z, x * y, fma(y, y, x * x));
-        else if (VARIANT == 2) v = (double)psi_f32((float)x, (float)y, (float)z, psi_f32_inv_scale(pd.k0));
+        else if (VARIANT == 2) v = (double)psi_f32((float)x, (float)y, (float)z, psi_f32_inv_scale(pd.k0), s_at);
         else {
             const PsiColumn pc = psi_column(x, y);
             v = pc.s * psi_eval<VARIANT == 3>(tb, pc, z);
