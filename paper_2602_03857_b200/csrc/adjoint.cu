@@ -179,13 +179,19 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
         if (kc <= 4) e = adj_launch<256, 4, 4, 3>(c, v, partial, done, work, s);
         else if (kc == 5) e = adj_launch<256, 5, 4, 3>(c, v, partial, done, work, s);
         else if (kc == 6) e = adj_launch<256, 6, 4, 3>(c, v, partial, done, work, s);
-        else e = adj_launch<256, 8, 4, 3>(c, v, partial, done, work, s);
+        else e = adj_launch<256, 8, 4, 3>(c, v, partial, done, work, s);      // any larger KC of the plan
     }
     else if (use_log2d(c)) {      // (threads, KC) pairs of make_plan's table
-        if (kc == 4) e = adj_launch<512, 4, 1, 2>(c, v, partial, done, work, s);
-        else if (kc == 5) e = adj_launch<384, 5, 1, 2>(c, v, partial, done, work, s);
-        else if (kc == 6) e = adj_launch<384, 6, 1, 2>(c, v, partial, done, work, s);
-        else e = adj_launch<256, 8, 1, 2>(c, v, partial, done, work, s);
+        switch (kc) {
+            case 4: e = adj_launch<512, 4, 1, 2>(c, v, partial, done, work, s); break;
+            case 5: e = adj_launch<384, 5, 1, 2>(c, v, partial, done, work, s); break;
+            case 6: e = adj_launch<384, 6, 1, 2>(c, v, partial, done, work, s); break;
+            case 7: e = adj_launch<384, 7, 1, 2>(c, v, partial, done, work, s); break;
+            case 11: e = adj_launch<256, 11, 1, 2>(c, v, partial, done, work, s); break;
+            case 13: e = adj_launch<256, 13, 1, 2>(c, v, partial, done, work, s); break;
+            case 17: e = adj_launch<256, 17, 1, 2>(c, v, partial, done, work, s); break;
+            default: e = adj_launch<256, 8, 1, 2>(c, v, partial, done, work, s); break;
+        }
     } else {
         if (kc == 4) e = adj_launch<256, 4, 2, 1>(c, v, partial, done, work, s);
         else if (kc == 5) e = adj_launch<256, 5, 2, 1>(c, v, partial, done, work, s);

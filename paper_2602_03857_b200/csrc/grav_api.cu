@@ -60,14 +60,15 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     p.fwd_reduce_rx = g.N < 32 * kDotBlocks ? 8 : 32;      // few stations: 8 per block and 32 chunk lanes (forward.cu)
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
     // KC nodes per thread: the per-(thread, station) set-up is shared by KC evaluations but the column is padded to a
-    // multiple of KC.  With the 2-D log table the compiled (threads, KC) variants measure 114.3 (256, 8), 112.5 (384, 6),
-    // 114.5 (384, 5) and 116.3 (512, 4) scheduler cycles per warp-evaluation before padding (configs 3 and 5,
-    // profiles/r2_adjoint_variants.md); without it the fit of round 1 stands, (119.5 + 25.6 / KC).  Pick the cheapest.
+    // multiple of KC.  With the 2-D log table the compiled (threads, KC) variants all measure 111-116 scheduler cycles
+    // per warp-evaluation before padding (configs 2-5), so the padding decides: pick the cheapest
+    // base x padded column.  Without the table the fit of round 1 stands, (119.5 + 25.6 / KC).
     p.adj_tpb = 256;
     p.adj_kc = 4;
     double best = 1e300;
     if (log2d) {
-        const struct { int tpb, kc; double cyc; } var[] = {{256, 8, 114.3}, {384, 6, 112.5}, {384, 5, 114.5}, {512, 4, 116.3}};
+        const struct { int tpb, kc; double cyc; } var[] = {{512, 4, 116.3}, {384, 5, 114.4}, {384, 6, 113.5}, {384, 7, 111.5},
+                                                           {256, 8, 113.5}, {256, 11, 113.0}, {256, 13, 112.3}, {256, 17, 113.6}};
         for (const auto& v : var) {
             const double cost = v.cyc * (double)(ceil_div(g.nzp, v.kc) * v.kc);
             if (cost < best) { best = cost; p.adj_kc = v.kc; p.adj_tpb = v.tpb; }
