@@ -215,6 +215,8 @@ def stored_g_leg(cfg, local, reps=5):
     ev = lambda: torch.cuda.Event(enable_timing=True)
     e0, e1 = ev(), ev()
     l0 = ctx.launches
+    ctx.store_g(fp32=fp32)                    # untimed first call (one-off shared-memory opt-in of the kernel on the host)
+    torch.cuda.synchronize()
     e0.record(); ctx.store_g(fp32=fp32); e1.record(); torch.cuda.synchronize()
     t_tab = e0.elapsed_time(e1)
 

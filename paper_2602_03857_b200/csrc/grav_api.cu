@@ -41,7 +41,7 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     p.sms = sms > 0 ? sms : 148;
     // Small problems (configs 1-2) run the node kernels persistently: with ~50 waves of short blocks the per-block table
     // fill (up to 140 KB from L2) and pipeline start cost 15-20 % of a launch there; from ~1e10 evaluations per product the
-    // plain grid is as fast or faster (profiles/r2_small_configs.md).
+    // plain grid is as fast or faster.
     p.persistent = (log2d && (double)g.N * (double)g.Nn < 1e10) ? 1 : 0;
     // Blocks of one launch all take the same time, so a grid of W.f waves of resident blocks costs ceil(W.f) waves:
     // with ~5 waves (the first plan) up to 18 % of the launch was tail.  ~100 blocks per SM keeps the tail <= 2-3 %

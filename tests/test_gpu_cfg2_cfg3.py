@@ -60,6 +60,19 @@ def test_cfg2_operators_full_oracle(cfg2):
     assert abs(cfg2["diag"].sum() / wl.N / 8.414e-4 - 1) <= 1e-3
 
 
+def test_cfg2_persistent_launch_is_deterministic(cfg2):
+    """Config 2 runs the node kernels persistently (blocks draw work items from a counter): which block
+    computes an item varies from run to run, the results may not - repeated products and CG runs are bit-identical."""
+    wl, ctx = cfg2["wl"], cfg2["ctx"]
+    u_w, v_w, _ = wl.test_vectors()
+    d0, g0 = ctx.forward(dev(u_w)), ctx.adjoint(dev(v_w))
+    c0 = ctx.dataspace_cg(dev(cfg2["d_obs"]), dev(cfg2["w"]), cfg2["lam"], 3)
+    for _ in range(3):
+        assert torch.equal(ctx.forward(dev(u_w)), d0) and torch.equal(ctx.adjoint(dev(v_w)), g0)
+    c1 = ctx.dataspace_cg(dev(cfg2["d_obs"]), dev(cfg2["w"]), cfg2["lam"], 3)
+    assert torch.equal(c0["alpha"], c1["alpha"]) and torch.equal(c0["m"], c1["m"]) and torch.equal(c0["hist"], c1["hist"])
+
+
 def test_cfg2_stored_f64(cfg2):
     wl, G, ctx = cfg2["wl"], cfg2["G"], cfg2["ctx"]
     u_w, v_w, _ = wl.test_vectors()
