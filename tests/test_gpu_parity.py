@@ -304,6 +304,36 @@ def test_launch_variants_against_oracle(shape):
     ctx.close()
 
 
+@pytest.mark.parametrize("shape", [(30, 34, 32, 1400), (26, 28, 50, 1500), (30, 26, 64, 1100), (10, 11, 150, 2800),
+                                   (44, 50, 20, 1300)])
+def test_default_paths_of_large_problems_on_midsize_shapes(shape):
+    """Problems just above 5e7 evaluations per product take the code paths of the large configs by DEFAULT - the 2-D log
+    table, the persistent launch, the (threads, KC) table of the adjoint: nz + 1 = 33, 51, 65, 151, 21 make make_plan
+    pick KC = 11, 17, 13, 7 (column padded to 154) and 7 - yet stay small enough for oracle rows and columns: forward on
+    sampled stations x all prisms, adjoint on sampled prisms (corners included) x all stations, Gram diagonal on sampled
+    stations, and bit-identical repeats."""
+    nx, ny, nz, nobs = shape
+    wl = workloads.make_custom(nx, ny, nz, 35.0, nobs, seed=nz, topo_amp=50.0)
+    assert wl.N * wl.n_nodes >= 5e7
+    mesh = oracle.Mesh(wl.xn, wl.yn, wl.zn)
+    rng = np.random.default_rng(nz)
+    u, v = rng.standard_normal(wl.M), rng.standard_normal(wl.N)
+    ctx = make_ctx(wl)
+    assert ctx.log2d_default
+    d, g = host(ctx.forward(dev(u))), host(ctx.adjoint(dev(v)))
+    st = rng.choice(wl.N, size=40, replace=False)
+    cells = np.unique(np.concatenate([rng.choice(wl.M, size=300, replace=False), [0, nz - 1, wl.M - nz, wl.M - 1]]))
+    d_ref = oracle.forward(mesh, wl.xo[st], wl.yo[st], wl.zo[st], wl.gamma, u)
+    g_ref = oracle.adjoint(mesh, wl.xo, wl.yo, wl.zo, wl.gamma, v, cells=cells)
+    assert np.abs(d[st] - d_ref).max() <= TOL_OP * np.abs(d).max()
+    assert np.abs(g[cells] - g_ref).max() <= TOL_OP * np.abs(g).max()
+    w = ctx.depth_weights(2.0, wl.z0)
+    G6 = oracle.tabulate(mesh, wl.xo[st[:6]], wl.yo[st[:6]], wl.zo[st[:6]], wl.gamma)
+    assert np.abs(host(ctx.gram_diag(w))[st[:6]] / oracle.gram_diag(G6, host(w)) - 1).max() <= 1e-10
+    assert np.array_equal(host(ctx.forward(dev(u))), d) and np.array_equal(host(ctx.adjoint(dev(v))), g)
+    ctx.close()
+
+
 def test_survey_coordinates_with_large_offsets():
     """UTM-like coordinates (x ~ 5e5 m, y ~ 4e6 m, mesh top 1,250 m below datum): the kernels work on corner-minus-station
     differences, the exponent offset k0 and the log-table range come from distances, not from the absolute coordinates."""
