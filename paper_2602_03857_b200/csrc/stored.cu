@@ -38,12 +38,11 @@ __host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPair
 // The difference buffer is double-buffered: every thread runs A(0), then per batch b: barrier, B(b) and A(b+1) - ONE
 // barrier per batch (B(b-1) precedes barrier b in every thread, so buffer (b+1)&1 is free after it).  Even warps run
 // B(b) first, odd warps A(b+1) first: the entry stores of one half overlap the FP64 work of the other.
-// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = with the 2-D log table.
+// EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table (see pair_dispatch for why not the 2-D one).
 // PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[station][tile].
 
-// Batch depth: 8 layers beside the 2-D log table (92-110 KB at the configs), 16 otherwise; compile-time so that the
-// entries of a thread live in registers.
-template <int EV> constexpr int pair_zb() { return EV == 2 ? 8 : 16; }
+// Batch depth in layers; compile-time so that the entries of a thread live in registers.
+template <int EV> constexpr int pair_zb() { return 16; }
 
 template <int MODE, int EV>
 __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev pd, int tnx, int tny, int tiles_y,
@@ -55,7 +54,6 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     PsiTabView tb;
     size_t tab_entries = 0;
     if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); tab_entries = (size_t)kTabEntries * kRep; }
-    if (EV == 2) { tb = psi_tables_to_smem_2d(s_tab, pd); tab_entries = psi_log2d_smem_entries(pd); }
     double* s_zn = reinterpret_cast<double*>(s_tab + tab_entries);
     double* s_d = s_zn + pair_zn_doubles(g.nzp);
     // node depths, the bottom node repeated so that phase A never has to clamp an index past the mesh bottom
@@ -87,7 +85,7 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
         auto eval = [&](double zn) -> double {
             const double Z = zn - zo;
             if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
-            return pc.s * psi_eval<EV == 2>(tb, pc, Z);
+            return pc.s * psi_eval<false>(tb, pc, Z);
         };
         const int d21 = nny * stride;
         // first entry of this thread's prism column in this station's row of G (element index fits 63 bits; the row
@@ -214,8 +212,8 @@ __global__ void gram_reduce_kernel(long long N, int ntiles, const double* __rest
 }
 
 static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev) {
-    const int zb = ev == 2 ? pair_zb<2>() : pair_zb<1>();
-    const size_t tab = ev == 0 ? 0 : (ev == 2 ? psi_smem_bytes<true>(pd) : kTabSmemBytes);
+    const int zb = pair_zb<1>();
+    const size_t tab = ev == 0 ? 0 : kTabSmemBytes;
     return tab + (size_t)pair_zn_doubles(g.nzp) * 8 + 2 * (size_t)kPairTPB * (zb + 2) * 8;   // double-buffered
 }
 constexpr size_t kPairSmemMax = 226 * 1024;     // dynamic part: the opt-in limit of 227 KB includes the static s_red
@@ -258,12 +256,14 @@ static cudaError_t pair_launch(grav_ctx* c, void* G, const double* w, double* gr
     return cudaGetLastError();
 }
 
+// The per-pair kernel always uses the 256-entry log table in 8 conflict-free copies, also where the matrix-free kernels
+// use the single-copy 2-D table: with the difference buffer's traffic on top of the look-ups it is bound by
+// shared-memory wavefronts, not by issue slots, so the table without bank collisions wins although it costs 2 FP64 + 7
+// other instructions more per evaluation (config 3 FP32 tabulation 103.7 -> 98.8 ms, Gram diagonal 120.3 -> 111.7 ms),
+// and its 66 KB leave room for batches of 16 layers.
 template <int MODE>
 static cudaError_t pair_dispatch(grav_ctx* c, void* G, const double* w, double* gram_partial, cudaStream_t s) {
     if (c->psi_variant == 1) return pair_launch<MODE, 0>(c, G, w, gram_partial, s);
-    // the 2-D log table only when it leaves room for the tile buffer
-    if (use_log2d(c) && pair_smem_bytes(c->g, c->pd, 2) <= kPairSmemMax)
-        return pair_launch<MODE, 2>(c, G, w, gram_partial, s);
     return pair_launch<MODE, 1>(c, G, w, gram_partial, s);
 }
 
