@@ -51,6 +51,11 @@ class Comm:
         self.world = dist.get_world_size(group) if dist.is_initialized() else 1
         self.rank = dist.get_rank(group) if dist.is_initialized() else 0
         self.calls = []           # ("allreduce" | "allgather", count) in call order
+        # CUDA buffers over a CPU-only backend (gloo): stage through host memory.  The copies synchronise the stream the
+        # library handed over, so the ordering with its kernels is kept; used to run two real ranks on ONE GPU in the
+        # tests (NCCL needs a device per rank), never by bench.py.
+        self.staged = (self.device.type == "cuda" and dist.is_initialized()
+                       and "nccl" not in str(dist.get_backend(group)).lower())
 
     def view(self, ptr: int, count: int) -> torch.Tensor:
         if self.device.type == "cuda":
@@ -68,13 +73,24 @@ class Comm:
 
     def allreduce_sum(self, ptr: int, count: int, stream: int = 0):
         with self._on(stream):
-            dist.all_reduce(self.view(ptr, count), op=dist.ReduceOp.SUM, group=self.group)
+            t = self.view(ptr, count)
+            if self.staged:
+                h = t.cpu()                                   # synchronises the stream
+                dist.all_reduce(h, op=dist.ReduceOp.SUM, group=self.group)
+                t.copy_(h)
+            else:
+                dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
         self.calls.append(("allreduce", count))
 
     def allgather(self, send_ptr: int, recv_ptr: int, count: int, stream: int = 0):
         with self._on(stream):
-            dist.all_gather_into_tensor(self.view(recv_ptr, count * self.world), self.view(send_ptr, count),
-                                        group=self.group)
+            recv, send = self.view(recv_ptr, count * self.world), self.view(send_ptr, count)
+            if self.staged:
+                parts = [torch.empty(count, dtype=torch.float64) for _ in range(self.world)]
+                dist.all_gather(parts, send.cpu(), group=self.group)
+                recv.copy_(torch.cat(parts))
+            else:
+                dist.all_gather_into_tensor(recv, send, group=self.group)
         self.calls.append(("allgather", count))
 
 

@@ -2,8 +2,10 @@
 model-space variables replicated and synchronised"): two NCCL ranks, each with the station shard
 of dist.ShardedContext and the exchange callbacks of dist.Comm, against the unsharded context on rank 0's device.
 
-Skipped on a box with fewer than 2 GPUs (the development pool's boxes have one; the CPU side of the same plumbing is
-tests/test_dist_cpu.py, the placement of the exchanges tests/test_gpu_parity.py::test_comm_exchange_placement).
+The NCCL test is skipped on a box with fewer than 2 GPUs (the development pool's boxes have one); there the second test
+runs the same two ranks on ONE GPU with gloo collectives staged through host memory (dist.Comm.staged), which exercises
+everything of the sharded product but NCCL itself.  (The CPU side of the plumbing is tests/test_dist_cpu.py, the
+placement of the exchanges tests/test_gpu_parity.py::test_comm_exchange_placement.)
 The workload is ragged and irregular (random stations over topography, the shape class of configs 4-5) and large
 enough that the adjoint's (hi, lo) planes matter: the sharded adjoint must agree with the single-rank one to 1e-10 of
 max (the operator tolerance), five CG iterates (prefix parity) and the recovered model to 1e-8."""
@@ -37,13 +39,16 @@ def _problem():
     return wl, rng.standard_normal(wl.N), rng.standard_normal(wl.M)
 
 
-def _worker(rank, world, port, out):
+def _worker(rank, world, port, out, backend="nccl"):
+    # backend "nccl": one device per rank.  "gloo": both ranks on cuda:0, the collectives staged through host memory by
+    # dist.Comm - two REAL ranks of the product (distinct shards, rank order, gather layout) on a one-GPU box; the ranks'
+    # kernels never wait on one another (the exchanges are host-driven, between launches).
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
-                      LOCAL_RANK=str(rank))
+                      LOCAL_RANK=str(rank if backend == "nccl" else 0))
     import torch.distributed as dist
     from paper_2602_03857_b200 import binding
     from paper_2602_03857_b200 import dist as gdist
-    r, w, local = gdist.init_from_env("nccl")
+    r, w, local = gdist.init_from_env(backend)
     try:
         torch.cuda.set_device(local)
         dev = torch.device("cuda", local)
@@ -58,6 +63,7 @@ def _worker(rank, world, port, out):
             wgt = ctx.depth_weights(2.0, wl.z0)
             # lambda from the global trace: each rank's Gram diagonal covers its own stations
             tr = ctx.gram_diag(wgt).sum().reshape(1)
+            tr = tr.cpu() if backend == "gloo" else tr              # the test's own collectives: host tensors under gloo
             dist.all_reduce(tr)
             lam = 1e-2 * float(tr.item()) / wl.N
             fwd = ctx.forward(to(u)) if mode == binding.MATRIX_FREE else ctx.forward_stored(to(u))
@@ -71,8 +77,9 @@ def _worker(rank, world, port, out):
                 adj_side = ctx.adjoint(sh.local(v)) if mode == binding.MATRIX_FREE else ctx.adjoint_stored(sh.local(v))
             side.synchronize()
             assert torch.equal(adj, adj_side)
-            gather = [torch.empty_like(adj) for _ in range(world)]
-            dist.all_gather(gather, adj)
+            mine = adj.cpu() if backend == "gloo" else adj
+            gather = [torch.empty_like(mine) for _ in range(world)]
+            dist.all_gather(gather, mine)
             assert all(torch.equal(gather[0], g) for g in gather), "replicated model-space vector differs between ranks"
             res[mode] = dict(lo=sh.lo, hi=sh.hi, lam=lam, fwd=fwd.cpu().numpy(), adj=adj.cpu().numpy(),
                              alpha=cg["alpha"].cpu().numpy(), m=cg["m"].cpu().numpy(), hist=cg["hist"].cpu().numpy(),
@@ -86,15 +93,26 @@ def _worker(rank, world, port, out):
 
 @pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs 2 GPUs (NCCL ranks on distinct devices)")
 def test_two_nccl_ranks_match_the_unsharded_context():
+    _run_two_ranks("nccl")
+
+
+@pytest.mark.skipif(not torch.cuda.is_available(), reason="needs a GPU")
+def test_two_ranks_on_one_gpu_match_the_unsharded_context():
+    """The same comparison with both ranks on cuda:0 and gloo collectives staged through host memory: what a one-GPU box
+    can verify of the sharded product - everything but NCCL itself."""
+    _run_two_ranks("gloo")
+
+
+def _run_two_ranks(backend):
     from paper_2602_03857_b200 import binding
     world = 2
     ctxmp = mp.get_context("spawn")
     out = ctxmp.Queue()
     port = _free_port()
-    procs = [ctxmp.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    procs = [ctxmp.Process(target=_worker, args=(r, world, port, out, backend)) for r in range(world)]
     for p in procs:
         p.start()
-    got = dict(out.get(timeout=600) for _ in range(world))
+    got = dict(out.get(timeout=300) for _ in range(world))
     for p in procs:
         p.join(timeout=120)
         assert p.exitcode == 0
