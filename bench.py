@@ -444,7 +444,12 @@ def run_ours(args):
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     if int(os.environ.get("WORLD_SIZE", "1")) > 1:
         os.environ.setdefault("NCCL_DEBUG", "INFO")       # rank / transport lines on stderr (the JSON line is stdout)
-    rank, world, local = gdist.init_from_env("nccl")
+    # NCCL, one rank per GPU.  GRAV_DIST_BACKEND=gloo (development only): several ranks share the visible GPUs and the
+    # collectives are staged through host memory (dist.Comm.staged) - a functional check of this file's multi-rank logic
+    # on a one-GPU box, never a measurement.
+    backend = os.environ.get("GRAV_DIST_BACKEND", "nccl")
+    rank, world, local = gdist.init_from_env(backend)
+    local %= torch.cuda.device_count()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     wl = workloads.make(args.config)
@@ -648,7 +653,7 @@ def run_ours(args):
     # per-rank kernel times (multi-GPU: the driver reads the spread)
     per_rank = None
     if world > 1:
-        t = torch.tensor([t_fwd, t_adj], dtype=torch.float64, device=dev)
+        t = torch.tensor([t_fwd, t_adj], dtype=torch.float64, device=dev if backend == "nccl" else "cpu")
         allt = [torch.empty_like(t) for _ in range(world)]
         torch.distributed.all_gather(allt, t)
         per_rank = [{"rank": r, "stations": gdist.shard_range(N, world, r)[1] - gdist.shard_range(N, world, r)[0],
