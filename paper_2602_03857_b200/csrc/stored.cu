@@ -18,30 +18,43 @@
 namespace grav {
 
 // ---- per-pair evaluation, node-shared --------------------------------------------------------------------
-constexpr int kPairTPB = 512;            // >= 22 x 23 node columns: 21 x 22 cell columns per tile
-constexpr int kPairWarps = kPairTPB / 32;
-constexpr int kPairU = 8;                // evaluations in flight per thread
-constexpr int kPairZPad = 32;             // bottom node repeated this many times behind the node depths in shared memory
+constexpr int kPairTPB = 512;            // threads per block: 12 producer warps + 4 consumer warps
+constexpr int kPairProd = 384;           // producer threads = node columns of a tile: up to 19 x 20 (18 x 19 cell columns)
+constexpr int kPairCons = kPairTPB - kPairProd;
+constexpr int kPairU = 8;                // evaluations in flight per producer thread
+constexpr int kPairZPad = 32;            // bottom node repeated this many times behind the node depths in shared memory
+constexpr int kPairMaxCells = 3;         // cell columns per consumer thread: (19 - 1) x (20 - 1) = 342 <= 3 x 128
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 __host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPairZPad + 1) & ~1; }
 
+// named barriers (0 is __syncthreads): FULL[b] - producers arrive, consumers wait; EMPTY[b] - consumers arrive, producers wait
+enum { BAR_FULL0 = 1, BAR_FULL1 = 2, BAR_EMPTY0 = 3, BAR_EMPTY1 = 4, BAR_CONS = 5 };
+__device__ __forceinline__ void bar_sync(int id, int count) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ void bar_arrive(int id, int count) {
+    __threadfence_block();
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+
 // Work item = (station, tile), tile index fastest; blocks stride over the items; the z-axis of an item is cut into
-// batches of zb layers.
-// Phase A(batch): thread t < nnx * nny owns node column (i0 + t / nny, j0 + t % nny): hoists once per item, then Psi down
-//   the column, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * stride + k - k0] (stride = zb + 2 doubles: 16-byte aligned
-//   rows whose 16-byte bank groups differ between neighbouring threads - conflict-free 128-bit accesses).
-// Phase B(batch): the thread of node column (la, lb) with la < ncx, lb < ncy also owns CELL column (la, lb): its zb
-//   entries are gamma * ((d11 - d21) - d12 + d22) from its own row of the buffer and the rows of threads t + 1, t + nny,
-//   t + nny + 1 - the same pairing as node_to_cell (vertical neighbours first: their Psi values are closest), so stored
-//   and matrix-free products agree to rounding.  zb independent entries per thread (no dependent chain), written as
-//   16-byte vector stores: every lane fills whole 32-byte sectors of its own prism column.
-// The difference buffer is double-buffered: every thread runs A(0), then per batch b: barrier, B(b) and A(b+1) - ONE
-// barrier per batch (B(b-1) precedes barrier b in every thread, so buffer (b+1)&1 is free after it).  Even warps run
-// B(b) first, odd warps A(b+1) first: the entry stores of one half overlap the FP64 work of the other.
+// batches of zb layers, numbered q = 0, 1, ... across the items of a block; batch q lives in buffer q & 1.
+// The block is warp-specialised.
+// Producers (warps 0-11): thread t < nnx * nny owns node column (i0 + t / nny, j0 + t % nny): hoists once per item, then
+//   Psi down the column, 8 evaluations in flight, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * stride + k - k0]
+//   (stride = zb + 2 doubles: 16-byte aligned rows whose 16-byte bank groups differ between neighbouring threads).
+//   Per batch: wait EMPTY[q & 1] (from q = 2 on), evaluate and store, arrive on FULL[q & 1].  They never touch G.
+// Consumers (warps 12-15): thread c owns cell columns c, c + 128, c + 256 of the tile.  Per batch: wait FULL[q & 1]; the
+//   zb entries of a cell column are gamma * ((d11 - d21) - d12 + d22) from the rows of its four corner columns - the
+//   same pairing as node_to_cell (vertical neighbours first: their Psi values are closest), so stored and matrix-free
+//   products agree to rounding - written as 16-byte vector stores (every lane fills whole 32-byte sectors of its own
+//   prism column); then arrive on EMPTY[q & 1].
+// So the FP64 pipe is fed by 3 warps per scheduler without interruption while the 4th turns differences into entries;
+// no block-wide barrier inside the item loop.
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table (see pair_dispatch for why not the 2-D one).
 // PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[station][tile].
 
-// Batch depth in layers; compile-time so that the entries of a thread live in registers.
+// Batch depth in layers; compile-time so that the entries of a cell column live in registers.
 template <int EV> constexpr int pair_zb() { return 16; }
 
 template <int MODE, int EV>
@@ -50,148 +63,165 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                                                                const double* __restrict__ winv2,
                                                                double* __restrict__ gram_partial) {
     extern __shared__ double2 s_tab[];
-    __shared__ double s_red[kPairWarps];
+    __shared__ double s_red[kPairCons / 32];
     PsiTabView tb;
     size_t tab_entries = 0;
     if (EV == 1) { tb = psi_tables_to_smem(s_tab, pd); tab_entries = (size_t)kTabEntries * kRep; }
     double* s_zn = reinterpret_cast<double*>(s_tab + tab_entries);
     double* s_d = s_zn + pair_zn_doubles(g.nzp);
-    // node depths, the bottom node repeated so that phase A never has to clamp an index past the mesh bottom
+    // node depths, the bottom node repeated so that the producers never have to clamp an index past the mesh bottom
     for (int c = threadIdx.x; c < g.nzp + kPairZPad; c += kPairTPB) s_zn[c] = g.zn[min(c, g.nz)];
     __syncthreads();
-    constexpr int zb = pair_zb<EV>(), stride = zb + 2, bufsz = kPairTPB * stride;
+    constexpr int zb = pair_zb<EV>(), stride = zb + 2, bufsz = kPairProd * stride;
     static_assert(zb % kPairU == 0 && kPairZPad >= zb, "batch = whole groups of evaluations; padding covers a batch");
-    const int t = threadIdx.x, warp = t >> 5;
+    const int t = threadIdx.x;
+    const bool producer = t < kPairProd;
     const int ds = (int)(gridDim.x / ntiles), dt = (int)(gridDim.x - ds * ntiles);  // item += gridDim.x as (station, tile)
     // 16-byte vector stores / loads need the prism columns 16-byte aligned in G: nz a multiple of 4 (FP32) or 2 (FP64)
     const bool vec_ok = MODE == PAIR_F32 ? (g.nz & 3) == 0 : (g.nz & 1) == 0;
+    const int nbatch = (g.nz + zb - 1) / zb;
+    // batches this block will process in all: the consumers skip the EMPTY arrivals nobody will wait for
+    const long long nitems = g.N * (long long)ntiles;
+    const long long my_items = blockIdx.x < nitems ? (nitems - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+    const long long total_batches = my_items * nbatch;
     long long st = blockIdx.x / ntiles;
     int tile = (int)(blockIdx.x - st * ntiles);
-    int par = 0;
-    for (; st < g.N; st += ds, tile += dt) {
+    long long q0 = 0;                                                    // number of the item's first batch
+    for (; st < g.N; st += ds, tile += dt, q0 += nbatch) {
         if (tile >= ntiles) { tile -= ntiles; if (++st >= g.N) break; }
         const int tx = tile / tiles_y, ty = tile - tx * tiles_y;
         const int i0 = tx * (tnx - 1), j0 = ty * (tny - 1);
         const int nnx = min(tnx, g.nxp - i0), nny = min(tny, g.nyp - j0);       // node columns of this tile
-        const bool active = t < nnx * nny;
-        const int la = active ? t / nny : 0, lb = active ? t - la * nny : 0;
-        const bool owns_cell = active && la < nnx - 1 && lb < nny - 1;          // cell column (la, lb) of this tile
-        const double xo = g.xo[st], yo = g.yo[st], zo = g.zo[st];
-        const double X = g.xn[i0 + la] - xo, Y = g.yn[j0 + lb] - yo;
-        PsiColumn pc;
-        double XY = 0.0, Q = 0.0;
-        if (EV != 0) pc = psi_column(X, Y);
-        else { XY = X * Y; Q = fma(Y, Y, X * X); }
-        auto eval = [&](double zn) -> double {
-            const double Z = zn - zo;
-            if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
-            return pc.s * psi_eval<false>(tb, pc, Z);
-        };
-        const int d21 = nny * stride;
-        // first entry of this thread's prism column in this station's row of G (element index fits 63 bits; the row
-        // base is kept opaque so that the compiler does not re-form st * M per store)
-        const int cell_first = ((i0 + la) * g.ny + j0 + lb) * g.nz;
-        size_t Grow = (size_t)Gout + (size_t)st * (size_t)g.M * (MODE == PAIR_F64 ? 8 : 4);
-        asm volatile("" : "+l"(Grow));
-        double prev = active ? eval(s_zn[0]) : 0.0;
-        double gram = 0.0;
-        auto phase_a = [&](int k0, double* buf) {
-            if (!active) return;
-            const int nb = min(zb, g.nz - k0);
-            double* dst = buf + t * stride;
-            // kPairU independent evaluations in flight; layers past the mesh bottom (last partial group only) are
-            // evaluated at the bottom node (s_zn is padded), stored, and never used
-            for (int kk = 0; kk < nb; kk += kPairU) {
-                const double* zp = s_zn + k0 + kk + 1;
-                double cur[kPairU];
+        const double zo = g.zo[st];
+        if (producer) {
+            const bool active = t < nnx * nny;
+            const int la = active ? t / nny : 0, lb = active ? t - la * nny : 0;
+            const double X = g.xn[i0 + la] - g.xo[st], Y = g.yn[j0 + lb] - g.yo[st];
+            PsiColumn pc;
+            double XY = 0.0, Q = 0.0;
+            if (EV != 0) pc = psi_column(X, Y);
+            else { XY = X * Y; Q = fma(Y, Y, X * X); }
+            auto eval = [&](double zn) -> double {
+                const double Z = zn - zo;
+                if (EV == 0) return psi_libm(X, Y, Z, XY, Q);
+                return pc.s * psi_eval<false>(tb, pc, Z);
+            };
+            double prev = active ? eval(s_zn[0]) : 0.0;
+            for (int b = 0; b < nbatch; ++b) {
+                const long long q = q0 + b;
+                const int par = (int)(q & 1);
+                if (q >= 2) bar_sync(BAR_EMPTY0 + par, kPairTPB);       // the consumers are done with batch q - 2
+                if (active) {
+                    const int k0 = b * zb, nb = min(zb, g.nz - k0);
+                    double* dst = s_d + par * bufsz + t * stride;
+                    // layers past the mesh bottom (last partial group only) are evaluated at the bottom node (s_zn is
+                    // padded), stored, and never used
+                    for (int kk = 0; kk < nb; kk += kPairU) {
+                        const double* zp = s_zn + k0 + kk + 1;
+                        double cur[kPairU];
 #pragma unroll
-                for (int u = 0; u < kPairU; ++u) cur[u] = eval(zp[u]);
+                        for (int u = 0; u < kPairU; ++u) cur[u] = eval(zp[u]);
 #pragma unroll
-                for (int u = 0; u < kPairU; u += 2)
-                    *reinterpret_cast<double2*>(dst + kk + u) =
-                        make_double2(cur[u] - (u ? cur[u - 1] : prev), cur[u + 1] - cur[u]);
-                prev = cur[kPairU - 1];
+                        for (int u = 0; u < kPairU; u += 2)
+                            *reinterpret_cast<double2*>(dst + kk + u) =
+                                make_double2(cur[u] - (u ? cur[u - 1] : prev), cur[u + 1] - cur[u]);
+                        prev = cur[kPairU - 1];
+                    }
+                }
+                bar_arrive(BAR_FULL0 + par, kPairTPB);
             }
-        };
-        auto phase_b = [&](int k0, const double* buf) {
-            if (!owns_cell) return;
-            const int nb = min(zb, g.nz - k0);
-            const double* p11 = buf + t * stride;
-            double val[zb];
+        } else {
+            const int ct = t - kPairProd;
+            const int ncy = nny - 1, ncells = (nnx - 1) * ncy;
+            // this thread's cell columns: offset of the (li, lj) row in a buffer, first entry of the prism column in G
+            int roff[kPairMaxCells], cell0[kPairMaxCells];
 #pragma unroll
-            for (int u = 0; u < zb; u += 2) {
-                const double2 a = *reinterpret_cast<const double2*>(p11 + u);
-                const double2 b = *reinterpret_cast<const double2*>(p11 + d21 + u);
-                const double2 c = *reinterpret_cast<const double2*>(p11 + stride + u);
-                const double2 d = *reinterpret_cast<const double2*>(p11 + d21 + stride + u);
-                val[u] = g.gamma * (((a.x - b.x) - c.x) + d.x);
-                val[u + 1] = g.gamma * (((a.y - b.y) - c.y) + d.y);
+            for (int m = 0; m < kPairMaxCells; ++m) {
+                const int cc = ct + m * kPairCons;
+                const int li = cc < ncells ? cc / ncy : 0, lj = cc < ncells ? cc - li * ncy : 0;
+                roff[m] = cc < ncells ? (li * nny + lj) * stride : -1;
+                cell0[m] = ((i0 + li) * g.ny + j0 + lj) * g.nz;
             }
-            const int cell = cell_first + k0;
-            if (MODE == PAIR_GRAM) {
-                if (nb == zb && vec_ok) {
+            const int d21 = nny * stride;
+            // (the row base is kept opaque so that the compiler does not re-form st * M per store)
+            size_t Grow = (size_t)Gout + (size_t)st * (size_t)g.M * (MODE == PAIR_F64 ? 8 : 4);
+            asm volatile("" : "+l"(Grow));
+            double gram = 0.0;
+            for (int b = 0; b < nbatch; ++b) {
+                const long long q = q0 + b;
+                const int par = (int)(q & 1);
+                const int k0 = b * zb, nb = min(zb, g.nz - k0);
+                bar_sync(BAR_FULL0 + par, kPairTPB);                    // the producers have stored batch q
+                const double* buf = s_d + par * bufsz;
+#pragma unroll
+                for (int m = 0; m < kPairMaxCells; ++m) {
+                    if (roff[m] < 0) continue;
+                    const double* p11 = buf + roff[m];
+                    double val[zb];
 #pragma unroll
                     for (int u = 0; u < zb; u += 2) {
-                        const double2 wi = __ldg(reinterpret_cast<const double2*>(winv2 + cell + u));
-                        gram = fma(val[u] * val[u], wi.x, gram);
-                        gram = fma(val[u + 1] * val[u + 1], wi.y, gram);
+                        const double2 a = *reinterpret_cast<const double2*>(p11 + u);
+                        const double2 bb = *reinterpret_cast<const double2*>(p11 + d21 + u);
+                        const double2 c = *reinterpret_cast<const double2*>(p11 + stride + u);
+                        const double2 d = *reinterpret_cast<const double2*>(p11 + d21 + stride + u);
+                        val[u] = g.gamma * (((a.x - bb.x) - c.x) + d.x);
+                        val[u + 1] = g.gamma * (((a.y - bb.y) - c.y) + d.y);
                     }
-                } else {
+                    const int cell = cell0[m] + k0;
+                    if (MODE == PAIR_GRAM) {
+                        if (nb == zb && vec_ok) {
 #pragma unroll
-                    for (int u = 0; u < zb; ++u)
-                        if (u < nb) gram = fma(val[u] * val[u], __ldg(winv2 + cell + u), gram);
+                            for (int u = 0; u < zb; u += 2) {
+                                const double2 wi = __ldg(reinterpret_cast<const double2*>(winv2 + cell + u));
+                                gram = fma(val[u] * val[u], wi.x, gram);
+                                gram = fma(val[u + 1] * val[u + 1], wi.y, gram);
+                            }
+                        } else {
+#pragma unroll
+                            for (int u = 0; u < zb; ++u)
+                                if (u < nb) gram = fma(val[u] * val[u], __ldg(winv2 + cell + u), gram);
+                        }
+                    } else if (MODE == PAIR_F64) {
+                        // (the opaque row address no longer tells the compiler its state space: say st.global)
+                        const size_t a0 = Grow + (size_t)cell * 8;
+                        if (nb == zb && vec_ok) {
+#pragma unroll
+                            for (int u = 0; u < zb; u += 2)
+                                asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(a0 + u * 8), "d"(val[u]), "d"(val[u + 1]));
+                        } else {
+#pragma unroll
+                            for (int u = 0; u < zb; ++u)
+                                if (u < nb) asm volatile("st.global.f64 [%0], %1;" ::"l"(a0 + u * 8), "d"(val[u]));
+                        }
+                    } else {
+                        const size_t a0 = Grow + (size_t)cell * 4;
+                        if (nb == zb && vec_ok) {
+#pragma unroll
+                            for (int u = 0; u < zb; u += 4)
+                                asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(a0 + u * 4), "f"((float)val[u]),
+                                             "f"((float)val[u + 1]), "f"((float)val[u + 2]), "f"((float)val[u + 3]));
+                        } else {
+#pragma unroll
+                            for (int u = 0; u < zb; ++u)
+                                if (u < nb) asm volatile("st.global.f32 [%0], %1;" ::"l"(a0 + u * 4), "f"((float)val[u]));
+                        }
+                    }
                 }
-            } else if (MODE == PAIR_F64) {
-                // (the opaque row address no longer tells the compiler its state space: say st.global)
-                const size_t a0 = Grow + (size_t)cell * 8;
-                if (nb == zb && vec_ok) {
+                if (q + 2 < total_batches) bar_arrive(BAR_EMPTY0 + par, kPairTPB);
+            }
+            if (MODE == PAIR_GRAM) {      // fixed-order sum over the consumer threads -> gram_partial[station][tile]
 #pragma unroll
-                    for (int u = 0; u < zb; u += 2)
-                        asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(a0 + u * 8), "d"(val[u]), "d"(val[u + 1]));
-                } else {
+                for (int o = 16; o > 0; o >>= 1) gram += __shfl_down_sync(0xffffffffu, gram, o);
+                if ((ct & 31) == 0) s_red[ct >> 5] = gram;
+                bar_sync(BAR_CONS, kPairCons);
+                if (ct == 0) {
+                    double sum = 0.0;
 #pragma unroll
-                    for (int u = 0; u < zb; ++u)
-                        if (u < nb) asm volatile("st.global.f64 [%0], %1;" ::"l"(a0 + u * 8), "d"(val[u]));
+                    for (int k = 0; k < kPairCons / 32; ++k) sum += s_red[k];
+                    gram_partial[st * ntiles + tile] = sum;
                 }
-            } else {
-                const size_t a0 = Grow + (size_t)cell * 4;
-                if (nb == zb && vec_ok) {
-#pragma unroll
-                    for (int u = 0; u < zb; u += 4)
-                        asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(a0 + u * 4), "f"((float)val[u]),
-                                     "f"((float)val[u + 1]), "f"((float)val[u + 2]), "f"((float)val[u + 3]));
-                } else {
-#pragma unroll
-                    for (int u = 0; u < zb; ++u)
-                        if (u < nb) asm volatile("st.global.f32 [%0], %1;" ::"l"(a0 + u * 4), "f"((float)val[u]));
-                }
+                bar_sync(BAR_CONS, kPairCons);
             }
-        };
-        const int nbatch = (g.nz + zb - 1) / zb;
-        phase_a(0, s_d + par * bufsz);
-        for (int b = 0; b < nbatch; ++b, par ^= 1) {
-            __syncthreads();
-            double* cur = s_d + par * bufsz;
-            double* nxt = s_d + (par ^ 1) * bufsz;
-            const bool more = b + 1 < nbatch;
-#pragma unroll 1
-            for (int ph = 0; ph < 2; ++ph) {
-                if ((ph == 0) == ((warp & 1) != 0)) { if (more) phase_a((b + 1) * zb, nxt); }
-                else phase_b(b * zb, cur);
-            }
-        }
-        if (MODE == PAIR_GRAM) {      // fixed-order block sum -> gram_partial[station][tile]
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) gram += __shfl_down_sync(0xffffffffu, gram, o);
-            if ((t & 31) == 0) s_red[warp] = gram;
-            __syncthreads();
-            if (t == 0) {
-                double sum = 0.0;
-#pragma unroll
-                for (int k = 0; k < kPairWarps; ++k) sum += s_red[k];
-                gram_partial[st * ntiles + tile] = sum;
-            }
-            __syncthreads();
         }
     }
 }
@@ -214,17 +244,17 @@ __global__ void gram_reduce_kernel(long long N, int ntiles, const double* __rest
 static size_t pair_smem_bytes(const Geom& g, const PsiDev& pd, int ev) {
     const int zb = pair_zb<1>();
     const size_t tab = ev == 0 ? 0 : kTabSmemBytes;
-    return tab + (size_t)pair_zn_doubles(g.nzp) * 8 + 2 * (size_t)kPairTPB * (zb + 2) * 8;   // double-buffered
+    return tab + (size_t)pair_zn_doubles(g.nzp) * 8 + 2 * (size_t)kPairProd * (zb + 2) * 8;   // double-buffered
 }
 constexpr size_t kPairSmemMax = 226 * 1024;     // dynamic part: the opt-in limit of 227 KB includes the static s_red
 
-// Tile shape: tnx * tny <= kPairTPB node columns minimising the number of tiles (every tile costs one block the same
+// Tile shape: tnx * tny <= kPairProd node columns minimising the number of tiles (every tile costs one block the same
 // time), ties towards the squarer tile.
 void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p) {
     long long best = -1;
     p.pair_tnx = p.pair_tny = 2;
-    for (int tnx = 2; tnx <= kPairTPB / 2; ++tnx) {
-        const int tny = kPairTPB / tnx;
+    for (int tnx = 2; tnx <= kPairProd / 2; ++tnx) {
+        const int tny = kPairProd / tnx;
         if (tny < 2) break;
         const int ex = tnx > g.nxp ? g.nxp : tnx, ey = tny > g.nyp ? g.nyp : tny;      // never larger than the mesh
         const long long tiles = (long long)((g.nx + ex - 2) / (ex - 1)) * ((g.ny + ey - 2) / (ey - 1));
