@@ -23,7 +23,6 @@ constexpr int kPairProd = 384;           // producer threads = node columns of a
 constexpr int kPairCons = kPairTPB - kPairProd;
 constexpr int kPairU = 8;                // evaluations in flight per producer thread
 constexpr int kPairZPad = 32;            // bottom node repeated this many times behind the node depths in shared memory
-constexpr int kPairMaxCells = 3;         // cell columns per consumer thread: (19 - 1) x (20 - 1) = 342 <= 3 x 128
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 __host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPairZPad + 1) & ~1; }
 
@@ -44,17 +43,18 @@ __device__ __forceinline__ void bar_arrive(int id, int count) {
 //   Psi down the column, 8 evaluations in flight, storing dPsi(k) = Psi(k+1) - Psi(k) at buf[t * stride + k - k0]
 //   (stride = zb + 2 doubles: 16-byte aligned rows whose 16-byte bank groups differ between neighbouring threads).
 //   Per batch: wait EMPTY[q & 1] (from q = 2 on), evaluate and store, arrive on FULL[q & 1].  They never touch G.
-// Consumers (warps 12-15): thread c owns cell columns c, c + 128, c + 256 of the tile.  Per batch: wait FULL[q & 1]; the
-//   zb entries of a cell column are gamma * ((d11 - d21) - d12 + d22) from the rows of its four corner columns - the
-//   same pairing as node_to_cell (vertical neighbours first: their Psi values are closest), so stored and matrix-free
-//   products agree to rounding - written as 16-byte vector stores (every lane fills whole 32-byte sectors of its own
-//   prism column); then arrive on EMPTY[q & 1].
+// Consumers (warps 12-15): lanes run along the layers of the batch: a warp takes 32 / zb neighbouring cell columns per
+//   trip, lane = (cell column within the trip, layer), the block kPairCons / zb cell columns per trip.  Per batch: wait
+//   FULL[q & 1]; an entry is gamma * ((d11 - d21) - d12 + d22) from the rows of its four corner columns - the same
+//   pairing as node_to_cell (vertical neighbours first: their Psi values are closest), so stored and matrix-free
+//   products agree to rounding - stored so that a warp writes runs of zb consecutive entries of G (whole 32-byte
+//   sectors); then arrive on EMPTY[q & 1].
 // So the FP64 pipe is fed by 3 warps per scheduler without interruption while the 4th turns differences into entries;
 // no block-wide barrier inside the item loop.
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table (see pair_dispatch for why not the 2-D one).
 // PAIR_GRAM: winv2[cell] = 1 / w_cell^2 (gram_winv2_kernel); the item's sum goes to gram_partial[station][tile].
 
-// Batch depth in layers; compile-time so that the entries of a cell column live in registers.
+// Batch depth in layers: compile-time, a power of two dividing 32 (the consumers' lane mapping).
 template <int EV> constexpr int pair_zb() { return 16; }
 
 template <int MODE, int EV>
@@ -77,8 +77,6 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     const int t = threadIdx.x;
     const bool producer = t < kPairProd;
     const int ds = (int)(gridDim.x / ntiles), dt = (int)(gridDim.x - ds * ntiles);  // item += gridDim.x as (station, tile)
-    // 16-byte vector stores / loads need the prism columns 16-byte aligned in G: nz a multiple of 4 (FP32) or 2 (FP64)
-    const bool vec_ok = MODE == PAIR_F32 ? (g.nz & 3) == 0 : (g.nz & 1) == 0;
     const int nbatch = (g.nz + zb - 1) / zb;
     // batches this block will process in all: the consumers skip the EMPTY arrivals nobody will wait for
     const long long nitems = g.N * (long long)ntiles;
@@ -131,18 +129,21 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 bar_arrive(BAR_FULL0 + par, kPairTPB);
             }
         } else {
+            // consumers: lanes along k.  A warp takes cpw = 32 / zb neighbouring cell columns per trip (flattened index
+            // cc = li * ncy + lj), lane = (cell within the trip, layer), so that its global accesses are runs of zb
+            // consecutive entries of G (64 bytes in FP32) instead of one 16-byte piece per lane
             const int ct = t - kPairProd;
+            constexpr int cpw = 32 / zb, trip = cpw * (kPairCons / 32);       // cell columns per warp trip / per block trip
+            const int l = ct & (zb - 1);
             const int ncy = nny - 1, ncells = (nnx - 1) * ncy;
-            // this thread's cell columns: offset of the (li, lj) row in a buffer, first entry of the prism column in G
-            int roff[kPairMaxCells], cell0[kPairMaxCells];
-#pragma unroll
-            for (int m = 0; m < kPairMaxCells; ++m) {
-                const int cc = ct + m * kPairCons;
-                const int li = cc < ncells ? cc / ncy : 0, lj = cc < ncells ? cc - li * ncy : 0;
-                roff[m] = cc < ncells ? (li * nny + lj) * stride : -1;
-                cell0[m] = ((i0 + li) * g.ny + j0 + lj) * g.nz;
-            }
+            const int cc_first = (ct >> 5) * cpw + ((ct & 31) / zb);
+            const int li_first = cc_first / ncy, lj_first = cc_first - li_first * ncy;
+            const int dli = trip / ncy, dlj = trip - dli * ncy;              // advance of (li, lj) per trip
             const int d21 = nny * stride;
+            const int off_first = (li_first * nny + lj_first) * stride, off_step = (dli * nny + dlj) * stride;
+            const int off_wrap = (nny - ncy) * stride;                       // lj -= ncy, li += 1
+            const int cell_first = ((i0 + li_first) * g.ny + j0 + lj_first) * g.nz + l;
+            const int cell_step = (dli * g.ny + dlj) * g.nz, cell_wrap = (g.ny - ncy) * g.nz;
             // (the row base is kept opaque so that the compiler does not re-form st * M per store)
             size_t Grow = (size_t)Gout + (size_t)st * (size_t)g.M * (MODE == PAIR_F64 ? 8 : 4);
             asm volatile("" : "+l"(Grow));
@@ -152,59 +153,26 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 const int par = (int)(q & 1);
                 const int k0 = b * zb, nb = min(zb, g.nz - k0);
                 bar_sync(BAR_FULL0 + par, kPairTPB);                    // the producers have stored batch q
-                const double* buf = s_d + par * bufsz;
-#pragma unroll
-                for (int m = 0; m < kPairMaxCells; ++m) {
-                    if (roff[m] < 0) continue;
-                    const double* p11 = buf + roff[m];
-                    double val[zb];
-#pragma unroll
-                    for (int u = 0; u < zb; u += 2) {
-                        const double2 a = *reinterpret_cast<const double2*>(p11 + u);
-                        const double2 bb = *reinterpret_cast<const double2*>(p11 + d21 + u);
-                        const double2 c = *reinterpret_cast<const double2*>(p11 + stride + u);
-                        const double2 d = *reinterpret_cast<const double2*>(p11 + d21 + stride + u);
-                        val[u] = g.gamma * (((a.x - bb.x) - c.x) + d.x);
-                        val[u + 1] = g.gamma * (((a.y - bb.y) - c.y) + d.y);
-                    }
-                    const int cell = cell0[m] + k0;
-                    if (MODE == PAIR_GRAM) {
-                        if (nb == zb && vec_ok) {
-#pragma unroll
-                            for (int u = 0; u < zb; u += 2) {
-                                const double2 wi = __ldg(reinterpret_cast<const double2*>(winv2 + cell + u));
-                                gram = fma(val[u] * val[u], wi.x, gram);
-                                gram = fma(val[u + 1] * val[u + 1], wi.y, gram);
-                            }
-                        } else {
-#pragma unroll
-                            for (int u = 0; u < zb; ++u)
-                                if (u < nb) gram = fma(val[u] * val[u], __ldg(winv2 + cell + u), gram);
-                        }
-                    } else if (MODE == PAIR_F64) {
+                const double* buf = s_d + par * bufsz + l;
+                if (l < nb) {
+                    // buffer offset and cell index advance with (li, lj): +step per trip, +wrap when lj wraps
+                    int lj = lj_first, off = off_first, cell = cell_first + k0;
+                    // 4 trips in flight in every mode.  (Measured for the Gram sum on config 3: 1 trip 167 ms, 2 104 ms,
+                    // 4 95 ms, 8 98 ms; parking the weights in shared memory ahead of the barrier, by plain or by
+                    // asynchronous copies, 100-103 ms: the kernel is bound by shared-memory wavefronts, not by the
+                    // latency of the weight loads.)
+#pragma unroll 4
+                    for (int cc = cc_first; cc < ncells; cc += trip) {
+                        double wi = 0.0;
+                        if (MODE == PAIR_GRAM) wi = __ldg(winv2 + cell);     // from L2: requested before the buffer is read
+                        const double* p11 = buf + off;
+                        const double val = g.gamma * (((p11[0] - p11[d21]) - p11[stride]) + p11[d21 + stride]);
                         // (the opaque row address no longer tells the compiler its state space: say st.global)
-                        const size_t a0 = Grow + (size_t)cell * 8;
-                        if (nb == zb && vec_ok) {
-#pragma unroll
-                            for (int u = 0; u < zb; u += 2)
-                                asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(a0 + u * 8), "d"(val[u]), "d"(val[u + 1]));
-                        } else {
-#pragma unroll
-                            for (int u = 0; u < zb; ++u)
-                                if (u < nb) asm volatile("st.global.f64 [%0], %1;" ::"l"(a0 + u * 8), "d"(val[u]));
-                        }
-                    } else {
-                        const size_t a0 = Grow + (size_t)cell * 4;
-                        if (nb == zb && vec_ok) {
-#pragma unroll
-                            for (int u = 0; u < zb; u += 4)
-                                asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(a0 + u * 4), "f"((float)val[u]),
-                                             "f"((float)val[u + 1]), "f"((float)val[u + 2]), "f"((float)val[u + 3]));
-                        } else {
-#pragma unroll
-                            for (int u = 0; u < zb; ++u)
-                                if (u < nb) asm volatile("st.global.f32 [%0], %1;" ::"l"(a0 + u * 4), "f"((float)val[u]));
-                        }
+                        if (MODE == PAIR_F64) asm volatile("st.global.f64 [%0], %1;" ::"l"(Grow + (size_t)cell * 8), "d"(val));
+                        else if (MODE == PAIR_F32) asm volatile("st.global.f32 [%0], %1;" ::"l"(Grow + (size_t)cell * 4), "f"((float)val));
+                        else gram = fma(val * val, wi, gram);
+                        lj += dlj; off += off_step; cell += cell_step;
+                        if (lj >= ncy) { lj -= ncy; off += off_wrap; cell += cell_wrap; }
                     }
                 }
                 if (q + 2 < total_batches) bar_arrive(BAR_EMPTY0 + par, kPairTPB);
