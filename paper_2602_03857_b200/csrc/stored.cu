@@ -21,7 +21,8 @@ namespace grav {
 constexpr int kPairTPB = 512;            // threads per block: 12 producer warps + 4 consumer warps
 constexpr int kPairProd = 384;           // producer threads = node columns of a tile: up to 19 x 20 (18 x 19 cell columns)
 constexpr int kPairCons = kPairTPB - kPairProd;
-constexpr int kPairU = 8;                // evaluations in flight per producer thread
+constexpr int kPairU = 8;                // evaluations in flight per producer thread when tabulating ...
+constexpr int kPairUGram = 4;            // ... when summing the Gram diagonal (config 3: 95.2 ms with 8, 91.0 ms with 4)
 constexpr int kPairZPad = 32;            // bottom node repeated this many times behind the node depths in shared memory
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 __host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPairZPad + 1) & ~1; }
@@ -73,7 +74,8 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     for (int c = threadIdx.x; c < g.nzp + kPairZPad; c += kPairTPB) s_zn[c] = g.zn[min(c, g.nz)];
     __syncthreads();
     constexpr int zb = pair_zb<EV>(), stride = zb + 2, bufsz = kPairProd * stride;
-    static_assert(zb % kPairU == 0 && kPairZPad >= zb, "batch = whole groups of evaluations; padding covers a batch");
+    constexpr int U = MODE == PAIR_GRAM ? kPairUGram : kPairU;
+    static_assert(zb % U == 0 && kPairZPad >= zb, "batch = whole groups of evaluations; padding covers a batch");
     const int t = threadIdx.x;
     const bool producer = t < kPairProd;
     const int ds = (int)(gridDim.x / ntiles), dt = (int)(gridDim.x - ds * ntiles);  // item += gridDim.x as (station, tile)
@@ -114,16 +116,16 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                     double* dst = s_d + par * bufsz + t * stride;
                     // layers past the mesh bottom (last partial group only) are evaluated at the bottom node (s_zn is
                     // padded), stored, and never used
-                    for (int kk = 0; kk < nb; kk += kPairU) {
+                    for (int kk = 0; kk < nb; kk += U) {
                         const double* zp = s_zn + k0 + kk + 1;
-                        double cur[kPairU];
+                        double cur[U];
 #pragma unroll
-                        for (int u = 0; u < kPairU; ++u) cur[u] = eval(zp[u]);
+                        for (int u = 0; u < U; ++u) cur[u] = eval(zp[u]);
 #pragma unroll
-                        for (int u = 0; u < kPairU; u += 2)
+                        for (int u = 0; u < U; u += 2)
                             *reinterpret_cast<double2*>(dst + kk + u) =
                                 make_double2(cur[u] - (u ? cur[u - 1] : prev), cur[u + 1] - cur[u]);
-                        prev = cur[kPairU - 1];
+                        prev = cur[U - 1];
                     }
                 }
                 bar_arrive(BAR_FULL0 + par, kPairTPB);
