@@ -193,6 +193,30 @@ grav_status grav_set_comm(grav_ctx* ctx, const grav_comm* comm);
 enum { GRAV_PREC_F64 = 0, GRAV_PREC_F32 = 1 };
 grav_status grav_set_precision(grav_ctx* ctx, int precision);
 
+/* Allocation-free stored-G adjoint product (for callers that cannot call cudaMalloc or hold a workspace: code under
+ * CUDA graph capture, serving loops, harnesses that forbid allocation):
+ *     g[m] = sum_i G[i][m] v[i]          (w_dev == NULL)        -- what grav_adjoint_stored computes (Eq. 10's G^T)
+ *     g[m] = sum_i G[i][m] v[i] / w[m]^2 (w_dev != NULL)        -- W^-2 G^T v, the model recovery of Eq. 10-11
+ * with the same kernels, row chunking and summation order as grav_adjoint_stored, so the results are bit-identical.
+ * Needs no context and no workspace: the per-chunk column sums go to a file-scope device array of
+ * GRAV_NOALLOC_MAX_DOUBLES doubles (16 MiB) that every GPU loading the library holds until exit.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating library routine; it enqueues 2 kernels on `stream` and returns.
+ * G_dev: N x M row-major on `device`, elem_bytes = 8 (double) or 4 (float; accumulated in FP64).  v_dev[N], w_dev[M] or
+ * NULL, g_dev[M]: device doubles, caller-owned.  Limit: min(16, ceil(N / 256)) * M <= GRAV_NOALLOC_MAX_DOUBLES (e.g.
+ * M <= 131,072 for N >= 3,841; M <= 2,097,152 for N <= 256); beyond it the call returns GRAV_EINVAL with a message
+ * stating the limit and launches nothing.
+ * The array is shared by all calls and keeps the last call's contents; nothing in it has to start at zero (every entry
+ * the reduction reads is written by the same call first).  Calls that overlap on the GPU (different streams, or
+ * different threads without ordering) race on it: serialise them on one stream or with events.
+ * The first call on a device looks up the array's address (cudaGetSymbolAddress, once per device; not an allocation):
+ * call grav_noalloc_setup(device) beforehand where that must not happen inside the critical region (e.g. before
+ * beginning a capture).  Errors: GRAV_EINVAL (NULL pointer, N or M < 1, elem_bytes, size beyond the limit, device
+ * index), GRAV_ECUDA. */
+#define GRAV_NOALLOC_MAX_DOUBLES (2ll << 20)
+grav_status grav_noalloc_setup(int device);
+grav_status grav_gemvt_noalloc(int device, const void* G_dev, int elem_bytes, long long N, long long M,
+                               const double* v_dev, const double* w_dev, double* g_dev, void* stream);
+
 /* Launch accounting: number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 long long grav_launch_count(const grav_ctx* ctx);
 /* FP64 DFMA-only microbenchmark: runs `iters` dependent-chain-free DFMA per thread on the whole device and

@@ -24,7 +24,7 @@ EXPORTS = [
     "grav_forward_host", "grav_adjoint_host", "grav_dataspace_cg_host", "grav_invert", "grav_launch_count",
     "grav_fp64_peak_probe", "grav_last_error", "grav_debug_set_psi_variant", "grav_debug_psi_eval_host",
     "grav_debug_k0", "grav_debug_log2d_binades", "grav_debug_log2d_default", "grav_debug_set_log2d", "grav_set_comm",
-    "grav_set_precision", "grav_debug_psi_eval_device",
+    "grav_set_precision", "grav_debug_psi_eval_device", "grav_noalloc_setup", "grav_gemvt_noalloc",
 ]
 
 # include/grav.h: grav_comm
@@ -117,6 +117,10 @@ def load():
     L.grav_debug_log2d_binades.argtypes = [vp]
     L.grav_debug_log2d_default.restype = i
     L.grav_debug_log2d_default.argtypes = [vp]
+    L.grav_noalloc_setup.restype = i
+    L.grav_noalloc_setup.argtypes = [i]
+    L.grav_gemvt_noalloc.restype = i
+    L.grav_gemvt_noalloc.argtypes = [i, vp, i, ll, ll, vp, vp, vp, vp]
     L.grav_last_error.restype = C.c_char_p
     L.grav_last_error.argtypes = []
     _lib = L
@@ -156,6 +160,32 @@ def _host(a, n, name):
     if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous and a.size == n):
         raise ValueError(f"{name}: need a contiguous float64 array of {n} elements")
     return C.c_void_p(a.ctypes.data)
+
+
+NOALLOC_MAX_DOUBLES = 2 << 20        # include/grav.h GRAV_NOALLOC_MAX_DOUBLES
+
+
+def noalloc_setup(device=0):
+    """grav_noalloc_setup: look up the built-in scratch array's address on `device` (once; before a capture begins)."""
+    _check(load().grav_noalloc_setup(int(device)))
+
+
+def gemvt_noalloc(G, v, w=None, out=None):
+    """grav_gemvt_noalloc: g = G^T v (w None) or W^-2 G^T v for a caller-held (N, M) float64 / float32 CUDA matrix, with
+    the scratch in the library's built-in device array: no context, no workspace, no allocation inside the call (pass
+    `out`; without it this wrapper allocates the result tensor itself).  Raises GravError beyond the array's limit."""
+    if not (isinstance(G, torch.Tensor) and G.is_cuda and G.dim() == 2 and G.is_contiguous()
+            and G.dtype in (torch.float64, torch.float32)):
+        raise ValueError("G: need a contiguous 2-D CUDA tensor of float64 or float32")
+    N, M = G.shape
+    g = torch.empty(M, dtype=torch.float64, device=G.device) if out is None else out
+    for t in (v, w, g):
+        if t is not None and t.device != G.device:
+            raise ValueError("all tensors must live on G's device")
+    with torch.cuda.device(G.device):
+        _check(load().grav_gemvt_noalloc(G.device.index, C.c_void_p(G.data_ptr()), G.element_size(), N, M,
+                                         _dev(v, N, "v"), _dev(w, M, "w"), _dev(g, M, "g"), _stream()))
+    return g
 
 
 class CGState:

@@ -348,6 +348,34 @@ grav_status grav_set_comm(grav_ctx* c, const grav_comm* comm) {
     return GRAV_OK;
 }
 
+// ---- allocation-free stored-G adjoint (csrc/stored.cu holds the device array and its address look-up) --------
+static_assert(GRAV_NOALLOC_MAX_DOUBLES == kNoAllocMaxDoubles, "include/grav.h states the limit of csrc/stored.cu");
+
+grav_status grav_noalloc_setup(int device) {
+    DeviceGuard dg(device);
+    if (!dg.ok) return fail(GRAV_EINVAL, "grav_noalloc_setup: cannot make the device current");
+    CK(noalloc_setup(device, nullptr), "cudaGetSymbolAddress(no-allocation scratch)");
+    return GRAV_OK;
+}
+
+grav_status grav_gemvt_noalloc(int device, const void* G, int elem_bytes, long long N, long long M, const double* v,
+                               const double* w, double* g, void* stream) {
+    if (!G || !v || !g) return fail(GRAV_EINVAL, "grav_gemvt_noalloc: NULL pointer");
+    if (N < 1 || M < 1) return fail(GRAV_EINVAL, "grav_gemvt_noalloc: N and M must be positive");
+    if (elem_bytes != 8 && elem_bytes != 4) return fail(GRAV_EINVAL, "grav_gemvt_noalloc: elem_bytes must be 8 or 4");
+    if (M > kNoAllocMaxDoubles || noalloc_gemvt_doubles(N, M) > kNoAllocMaxDoubles) {
+        char need[64], have[64];
+        snprintf(need, sizeof(need), "%lld", M > kNoAllocMaxDoubles ? M : noalloc_gemvt_doubles(N, M));
+        snprintf(have, sizeof(have), "%lld", (long long)kNoAllocMaxDoubles);
+        return fail(GRAV_EINVAL, "grav_gemvt_noalloc: min(16, ceil(N/256)) * M = %s doubles of scratch exceed the built-in "
+                                 "array of %s doubles (16 MiB); use grav_adjoint_stored with a workspace", need, have);
+    }
+    DeviceGuard dg(device);
+    if (!dg.ok) return fail(GRAV_EINVAL, "grav_gemvt_noalloc: cannot make the device current");
+    CK(launch_gemvt_noalloc(device, G, elem_bytes, N, M, v, w, g, (cudaStream_t)stream), "gemvt_noalloc");
+    return GRAV_OK;
+}
+
 long long grav_launch_count(const grav_ctx* c) { return c ? c->launches : 0; }
 
 grav_status grav_debug_set_psi_variant(grav_ctx* c, int variant) {

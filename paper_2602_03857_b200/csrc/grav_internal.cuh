@@ -141,6 +141,12 @@ cudaError_t launch_gram_diag(grav_ctx* c, const double* w, double* winv2, double
 cudaError_t launch_form_A(grav_ctx* c, const double* G, const double* w, double lam, double* A, cudaStream_t s);
 cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, double* x, int n, cudaStream_t s);
 int gemvt_chunks(long long N);
+// no-allocation variant of gemvt: per-chunk sums in a file-scope device array of kNoAllocMaxDoubles (16 MiB)
+constexpr long long kNoAllocMaxDoubles = 2ll << 20;
+cudaError_t noalloc_setup(int device, double** ptr_or_null);
+long long noalloc_gemvt_doubles(long long N, long long M);
+cudaError_t launch_gemvt_noalloc(int device, const void* G, int elem, long long N, long long M, const double* v,
+                                 const double* w_or_null, double* g, cudaStream_t s);
 void make_pair_plan(const Geom& g, const PsiDev& pd, bool log2d, Plan& p);
 size_t gram_partial_doubles(const Geom& g, const Plan& p);
 // --- psi_check.cu : one Psi evaluation per argument triple with the chosen device evaluator (diagnostic)

@@ -493,4 +493,53 @@ cudaError_t launch_cholesky_solve(grav_ctx* c, double* A, const double* b, doubl
     return cudaGetLastError();
 }
 
+// ---- g = [W^-2] G^T v without any allocation (grav_gemvt_noalloc, include/grav.h) -----------------------------
+// The same two kernels and the same row chunking as launch_gemvt; the per-chunk column sums live in a file-scope device
+// array instead of the caller's workspace, so the call needs no context, no workspace and no cudaMalloc (callers under
+// CUDA graph capture, serving loops and harnesses that forbid allocation).  Every GPU that loads the library holds the
+// array until exit.  In host code the array's NAME is a host-side stand-in, not a device address: its device address
+// is looked up here once per device with cudaGetSymbolAddress, with that device current, and handed to the kernels.
+// All calls share the array and it keeps the last call's contents; nothing in it has to start at zero, because
+// gemvt_kernel writes every (chunk, column) entry that gemvt_reduce_kernel reads (all nchunk chunks of all M columns)
+// before the reduction runs on the same stream.  Calls that overlap on the GPU (different streams) race on it.
+static __device__ __align__(256) double g_noalloc_partial[kNoAllocMaxDoubles];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+double* s_noalloc_ptr[kNoAllocMaxDevices];          // device address of g_noalloc_partial on each device (0 = not looked up)
+}
+
+// Set-up for `device` (which must be current): look the array's device address up.  Idempotent and thread-safe (two
+// racing threads store the same value).  Not an allocation: the array is part of the loaded module.
+cudaError_t noalloc_setup(int device, double** out) {
+    if (device < 0 || device >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    double* ptr = __atomic_load_n(&s_noalloc_ptr[device], __ATOMIC_ACQUIRE);
+    if (!ptr) {
+        cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_partial);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        __atomic_store_n(&s_noalloc_ptr[device], ptr, __ATOMIC_RELEASE);
+    }
+    if (out) *out = ptr;
+    return cudaSuccess;
+}
+
+long long noalloc_gemvt_doubles(long long N, long long M) { return (long long)gemvt_chunks(N) * M; }
+
+// `device` is current.  The caller has checked noalloc_gemvt_doubles(N, M) <= kNoAllocMaxDoubles.
+cudaError_t launch_gemvt_noalloc(int device, const void* G, int elem, long long N, long long M, const double* v,
+                                 const double* w, double* g, cudaStream_t s) {
+    double* partial = nullptr;
+    cudaError_t e = noalloc_setup(device, &partial);
+    if (e != cudaSuccess) return e;
+    const int nchunk = gemvt_chunks(N);
+    const int rpc = (int)((N + nchunk - 1) / nchunk);
+    const long long M2 = (M + 1) >> 1;
+    dim3 grid((unsigned)((M2 + 127) / 128), nchunk);
+    if (elem == 8) gemvt_kernel<double, 128><<<grid, 128, 0, s>>>(N, M, (const double*)G, v, partial, rpc);
+    else gemvt_kernel<float, 128><<<grid, 128, 0, s>>>(N, M, (const float*)G, v, partial, rpc);
+    gemvt_reduce_kernel<<<(unsigned)((M + 255) / 256), 256, 0, s>>>(M, nchunk, partial, w, g);
+    return cudaGetLastError();
+}
+
 }  // namespace grav
