@@ -21,9 +21,11 @@ namespace grav {
 constexpr int kPairTPB = 512;            // threads per block: 12 producer warps + 4 consumer warps
 constexpr int kPairProd = 384;           // producer threads = node columns of a tile: up to 19 x 20 (18 x 19 cell columns)
 constexpr int kPairCons = kPairTPB - kPairProd;
-constexpr int kPairU = 8;                // evaluations in flight per producer thread when tabulating ...
-constexpr int kPairUGram = 4;            // ... when summing the Gram diagonal (config 3: 95.2 ms with 8, 91.0 ms with 4)
+constexpr int kPairU = 16;               // evaluations in flight per producer thread when tabulating ...
+constexpr int kPairUGram = 8;            // ... when summing the Gram diagonal
 constexpr int kPairZPad = 32;            // bottom node repeated this many times behind the node depths in shared memory
+// registers per thread after the hand-over from the consumer warpgroup to the producers: 384 x 144 + 128 x 80 = 512 x 128
+constexpr int kPairConsRegs = 80, kPairProdRegs = 144;
 enum { PAIR_F64 = 0, PAIR_F32 = 1, PAIR_GRAM = 2 };
 __host__ __device__ constexpr int pair_zn_doubles(int nzp) { return (nzp + kPairZPad + 1) & ~1; }
 
@@ -84,19 +86,30 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
     const long long nitems = g.N * (long long)ntiles;
     const long long my_items = blockIdx.x < nitems ? (nitems - 1 - blockIdx.x) / gridDim.x + 1 : 0;
     const long long total_batches = my_items * nbatch;
-    long long st = blockIdx.x / ntiles;
-    int tile = (int)(blockIdx.x - st * ntiles);
-    long long q0 = 0;                                                    // number of the item's first batch
-    for (; st < g.N; st += ds, tile += dt, q0 += nbatch) {
-        if (tile >= ntiles) { tile -= ntiles; if (++st >= g.N) break; }
+    // The block's items in order; both roles walk them with the same arithmetic.
+    struct Item { long long st; int tile, i0, j0, nnx, nny; };
+    auto item_at = [&](long long st, int tile) {
         const int tx = tile / tiles_y, ty = tile - tx * tiles_y;
         const int i0 = tx * (tnx - 1), j0 = ty * (tny - 1);
-        const int nnx = min(tnx, g.nxp - i0), nny = min(tny, g.nyp - j0);       // node columns of this tile
-        const double zo = g.zo[st];
-        if (producer) {
-            const bool active = t < nnx * nny;
-            const int la = active ? t / nny : 0, lb = active ? t - la * nny : 0;
-            const double X = g.xn[i0 + la] - g.xo[st], Y = g.yn[j0 + lb] - g.yo[st];
+        return Item{st, tile, i0, j0, min(tnx, g.nxp - i0), min(tny, g.nyp - j0)};      // node columns of this tile
+    };
+    // The two roles run the item loop in separate branches, each with its own loop variables (sharing them across the
+    // branches costs 11 % at config 3), so that each is compiled against its own register budget:
+    // when tabulating, registers move from the consumer warpgroup to the three producer warpgroups (whole warpgroups,
+    // once; config 3 FP32 tabulation 88.1 -> 85.8 ms.  The Gram sum's consumers want their registers: 89.2 ms without
+    // the hand-over, 92.6-94.5 ms with it).
+    if (producer) {
+        if (MODE != PAIR_GRAM) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kPairProdRegs));
+        long long st = blockIdx.x / ntiles;
+        int tile = (int)(blockIdx.x - st * ntiles);
+        long long q0 = 0;                                                        // number of the item's first batch
+        for (; st < g.N; st += ds, tile += dt, q0 += nbatch) {
+            if (tile >= ntiles) { tile -= ntiles; if (++st >= g.N) break; }
+            const Item it = item_at(st, tile);
+            const double zo = g.zo[st];
+            const bool active = t < it.nnx * it.nny;
+            const int la = active ? t / it.nny : 0, lb = active ? t - la * it.nny : 0;
+            const double X = g.xn[it.i0 + la] - g.xo[st], Y = g.yn[it.j0 + lb] - g.yo[st];
             PsiColumn pc;
             double XY = 0.0, Q = 0.0;
             if (EV != 0) pc = psi_column(X, Y);
@@ -110,7 +123,7 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
             for (int b = 0; b < nbatch; ++b) {
                 const long long q = q0 + b;
                 const int par = (int)(q & 1);
-                if (q >= 2) bar_sync(BAR_EMPTY0 + par, kPairTPB);       // the consumers are done with batch q - 2
+                if (q >= 2) bar_sync(BAR_EMPTY0 + par, kPairTPB);           // the consumers are done with batch q - 2
                 if (active) {
                     const int k0 = b * zb, nb = min(zb, g.nz - k0);
                     double* dst = s_d + par * bufsz + t * stride;
@@ -130,21 +143,29 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 }
                 bar_arrive(BAR_FULL0 + par, kPairTPB);
             }
-        } else {
-            // consumers: lanes along k.  A warp takes cpw = 32 / zb neighbouring cell columns per trip (flattened index
-            // cc = li * ncy + lj), lane = (cell within the trip, layer), so that its global accesses are runs of zb
-            // consecutive entries of G (64 bytes in FP32) instead of one 16-byte piece per lane
-            const int ct = t - kPairProd;
-            constexpr int cpw = 32 / zb, trip = cpw * (kPairCons / 32);       // cell columns per warp trip / per block trip
-            const int l = ct & (zb - 1);
-            const int ncy = nny - 1, ncells = (nnx - 1) * ncy;
-            const int cc_first = (ct >> 5) * cpw + ((ct & 31) / zb);
+        }
+    } else {
+        if (MODE != PAIR_GRAM) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kPairConsRegs));
+        long long st = blockIdx.x / ntiles;
+        int tile = (int)(blockIdx.x - st * ntiles);
+        long long q0 = 0;                                                        // number of the item's first batch
+        // consumers: lanes along k.  A warp takes cpw = 32 / zb neighbouring cell columns per trip (flattened index
+        // cc = li * ncy + lj), lane = (cell within the trip, layer), so that its global accesses are runs of zb
+        // consecutive entries of G (64 bytes in FP32) instead of one 16-byte piece per lane
+        const int ct = t - kPairProd;
+        constexpr int cpw = 32 / zb, trip = cpw * (kPairCons / 32);           // cell columns per warp trip / per block trip
+        const int l = ct & (zb - 1);
+        const int cc_first = (ct >> 5) * cpw + ((ct & 31) / zb);
+        for (; st < g.N; st += ds, tile += dt, q0 += nbatch) {
+            if (tile >= ntiles) { tile -= ntiles; if (++st >= g.N) break; }
+            const Item it = item_at(st, tile);
+            const int nny = it.nny, ncy = nny - 1, ncells = (it.nnx - 1) * ncy;
             const int li_first = cc_first / ncy, lj_first = cc_first - li_first * ncy;
             const int dli = trip / ncy, dlj = trip - dli * ncy;              // advance of (li, lj) per trip
             const int d21 = nny * stride;
             const int off_first = (li_first * nny + lj_first) * stride, off_step = (dli * nny + dlj) * stride;
             const int off_wrap = (nny - ncy) * stride;                       // lj -= ncy, li += 1
-            const int cell_first = ((i0 + li_first) * g.ny + j0 + lj_first) * g.nz + l;
+            const int cell_first = ((it.i0 + li_first) * g.ny + it.j0 + lj_first) * g.nz + l;
             const int cell_step = (dli * g.ny + dlj) * g.nz, cell_wrap = (g.ny - ncy) * g.nz;
             // (the row base is kept opaque so that the compiler does not re-form st * M per store)
             size_t Grow = (size_t)Gout + (size_t)st * (size_t)g.M * (MODE == PAIR_F64 ? 8 : 4);
@@ -154,15 +175,14 @@ __global__ void __launch_bounds__(kPairTPB, 1) pair_tile_kernel(Geom g, PsiDev p
                 const long long q = q0 + b;
                 const int par = (int)(q & 1);
                 const int k0 = b * zb, nb = min(zb, g.nz - k0);
-                bar_sync(BAR_FULL0 + par, kPairTPB);                    // the producers have stored batch q
+                bar_sync(BAR_FULL0 + par, kPairTPB);                        // the producers have stored batch q
                 const double* buf = s_d + par * bufsz + l;
                 if (l < nb) {
                     // buffer offset and cell index advance with (li, lj): +step per trip, +wrap when lj wraps
                     int lj = lj_first, off = off_first, cell = cell_first + k0;
                     // 4 trips in flight in every mode.  (Measured for the Gram sum on config 3: 1 trip 167 ms, 2 104 ms,
                     // 4 95 ms, 8 98 ms; parking the weights in shared memory ahead of the barrier, by plain or by
-                    // asynchronous copies, 100-103 ms: the kernel is bound by shared-memory wavefronts, not by the
-                    // latency of the weight loads.)
+                    // asynchronous copies, 100-103 ms.)
 #pragma unroll 4
                     for (int cc = cc_first; cc < ncells; cc += trip) {
                         double wi = 0.0;
