@@ -23,12 +23,85 @@ constexpr int kAdjObsTile = 256;
 
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table,
 // 3 = the Float32 evaluator psi_f32 with FP64 accumulation (grav_set_precision)
+//
+// One item = one block of TPB threads x one station chunk: thread t of node-thread block bx owns the K nodes
+// zbeg + cg K ... of node column col, (cg, col) = (t / ncol, t % ncol), t < ncol * ncg.
+template <int TPB, int K, int EV>
+__device__ __forceinline__ void adjoint_item(const Geom& g, const PsiTabView& tb, const float* s_at, float inv_scale,
+                                             double4* s_obs, const double* __restrict__ v, double* __restrict__ partial,
+                                             int bx, int by, int zbeg, int ncg, int obs_per_chunk) {
+    const long long nthreads = (long long)g.ncol * ncg;
+    const long long t = (long long)bx * TPB + threadIdx.x;
+    const bool valid = t < nthreads;
+    const long long tl = valid ? t : nthreads - 1;
+    const int cg = (int)(tl / g.ncol);        // column index fastest: lanes of a warp are neighbouring columns
+    const int col = (int)(tl - (long long)cg * g.ncol);
+    const int a = col / g.nyp, b = col - a * g.nyp;
+    const int c0 = zbeg + cg * K;
+    const double xa = g.xn[a], yb = g.yn[b];
+    double zc[K], acc[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        zc[k] = g.zn[min(c0 + k, g.nzp - 1)];
+        acc[k] = 0.0;
+    }
+    const long long i0 = (long long)by * obs_per_chunk;
+    const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
+    double* out_hi = partial + (long long)by * 2 * g.Nn + (long long)col * g.nzp + c0;
+    double* out_lo = out_hi + g.Nn;
+    for (long long base = i0; base < i1; base += kAdjObsTile) {
+        const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
+        __syncthreads();
+        for (int j = threadIdx.x; j < cnt; j += TPB)
+            s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
+        __syncthreads();
+        for (int j = 0; j < cnt; ++j) {
+            const double4 o = s_obs[j];
+            const double X = xa - o.x, Y = yb - o.y;
+            if (EV == 1 || EV == 2) {
+                const PsiColumn pc = psi_column(X, Y);
+                const double vs = o.w * pc.s;
+#pragma unroll
+                for (int k = 0; k < K; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
+            } else if (EV == 3) {
+                const float Xf = (float)X, Yf = (float)Y;
+#pragma unroll
+                for (int k = 0; k < K; ++k)
+                    acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale, s_at), acc[k]);
+            } else {
+                const double XY = X * Y;
+                const double Q = fma(Y, Y, X * X);
+#pragma unroll
+                for (int k = 0; k < K; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
+            }
+        }
+        // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
+        if (valid) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                if (c0 + k < g.nzp) {
+                    double hi = acc[k], lo = 0.0;
+                    if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
+                    out_hi[k] = hi;
+                    out_lo[k] = lo;
+                }
+                acc[k] = 0.0;
+            }
+        }
+    }
+}
+
+// KT > 0: the column is cut into ncg_main groups of KC nodes and ONE tail group of KT nodes (the nodes from
+// ncg_main * KC on), instead of padding the last group of KC: node-thread blocks bx < nblocks_main run the KC body,
+// the others the KT body (prime column lengths - config 5 has 151 nodes - otherwise pay up to KC - 1 wasted
+// evaluations per column and station).  KT = 0: ncg_main groups of KC cover the column, the last one padded.
 // work != NULL: persistent launch for small problems (see forward.cu): the block fills the tables once and draws
 // (node-thread block, station chunk) items from the counter.
-template <int TPB, int KC, int MINB, int EV>
+template <int TPB, int KC, int MINB, int EV, int KT>
 __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev pd, const double* __restrict__ v,
-                                                                  double* __restrict__ partial, int ncg,
-                                                                  int obs_per_chunk, const int* __restrict__ done,
+                                                                  double* __restrict__ partial, int ncg_main,
+                                                                  int nblocks_main, int obs_per_chunk,
+                                                                  const int* __restrict__ done,
                                                                   int* __restrict__ work, int nblocks, int nitems) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
@@ -39,7 +112,6 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
     if (EV == 1 || EV == 2) tb = psi_tables_load<EV == 2>(s_tab, pd);
     if (EV == 3) psi_f32_atan_table(s_at, pd);
     const float inv_scale = psi_f32_inv_scale(pd.k0);
-    const long long nthreads = (long long)g.ncol * ncg;
     for (;;) {
         int bx = blockIdx.x, by = blockIdx.y;
         if (work) {
@@ -51,64 +123,11 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
             by = item / nblocks;                         // node block fastest: neighbours in time share a station chunk
             bx = item - by * nblocks;
         }
-        const long long t = (long long)bx * TPB + threadIdx.x;
-        const bool valid = t < nthreads;
-        const long long tl = valid ? t : nthreads - 1;
-        const int cg = (int)(tl / g.ncol);        // column index fastest: lanes of a warp are neighbouring columns
-        const int col = (int)(tl - (long long)cg * g.ncol);
-        const int a = col / g.nyp, b = col - a * g.nyp;
-        const int c0 = cg * KC;
-        const double xa = g.xn[a], yb = g.yn[b];
-        double zc[KC], acc[KC];
-#pragma unroll
-        for (int k = 0; k < KC; ++k) {
-            zc[k] = g.zn[min(c0 + k, g.nzp - 1)];
-            acc[k] = 0.0;
-        }
-        const long long i0 = (long long)by * obs_per_chunk;
-        const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
-        double* out_hi = partial + (long long)by * 2 * g.Nn + (long long)col * g.nzp + c0;
-        double* out_lo = out_hi + g.Nn;
-        for (long long base = i0; base < i1; base += kAdjObsTile) {
-            const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
-            __syncthreads();
-            for (int j = threadIdx.x; j < cnt; j += TPB)
-                s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
-            __syncthreads();
-            for (int j = 0; j < cnt; ++j) {
-                const double4 o = s_obs[j];
-                const double X = xa - o.x, Y = yb - o.y;
-                if (EV == 1 || EV == 2) {
-                    const PsiColumn pc = psi_column(X, Y);
-                    const double vs = o.w * pc.s;
-#pragma unroll
-                    for (int k = 0; k < KC; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
-                } else if (EV == 3) {
-                    const float Xf = (float)X, Yf = (float)Y;
-#pragma unroll
-                    for (int k = 0; k < KC; ++k)
-                        acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale, s_at), acc[k]);
-                } else {
-                    const double XY = X * Y;
-                    const double Q = fma(Y, Y, X * X);
-#pragma unroll
-                    for (int k = 0; k < KC; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
-                }
-            }
-            // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
-            if (valid) {
-#pragma unroll
-                for (int k = 0; k < KC; ++k) {
-                    if (c0 + k < g.nzp) {
-                        double hi = acc[k], lo = 0.0;
-                        if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
-                        out_hi[k] = hi;
-                        out_lo[k] = lo;
-                    }
-                    acc[k] = 0.0;
-                }
-            }
-        }
+        if (KT == 0 || bx < nblocks_main)
+            adjoint_item<TPB, KC, EV>(g, tb, s_at, inv_scale, s_obs, v, partial, bx, by, 0, ncg_main, obs_per_chunk);
+        else
+            adjoint_item<TPB, (KT > 0 ? KT : 1), EV>(g, tb, s_at, inv_scale, s_obs, v, partial, bx - nblocks_main, by,
+                                                     ncg_main * KC, 1, obs_per_chunk);
         if (!work) break;
     }
 }
@@ -140,20 +159,21 @@ __global__ void adjoint_reduce_kernel(long long Nn, int nchunk, const double* __
     tnode[Nn + n] = lo;
 }
 
-template <int TPB, int KC, int MINB, int EV>
+template <int TPB, int KC, int MINB, int EV, int KT = 0>
 static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, const int* done, int* work,
                               cudaStream_t s) {
     // the opt-in is sized for the largest 2-D table, the launch for this context's table
     const size_t smem = (EV == 1 || EV == 2) ? psi_smem_bytes<EV == 2>(c->pd) : 0;
     static unsigned long long smem_set = 0;
     if (EV == 1 || EV == 2) {
-        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV>, psi_smem_max<EV == 2>(), c->device,
-                                            &smem_set);
+        cudaError_t e = ensure_dynamic_smem(adjoint_nodes_kernel<TPB, KC, MINB, EV, KT>, psi_smem_max<EV == 2>(),
+                                            c->device, &smem_set);
         if (e != cudaSuccess) return e;
     }
-    const int ncg = (c->g.nzp + KC - 1) / KC;
-    const long long nthreads = (long long)c->g.ncol * ncg;
-    const int nblocks = (int)((nthreads + TPB - 1) / TPB);
+    // KT > 0: whole groups of KC, then one tail group of KT covering the rest of the column (make_plan guarantees it does)
+    const int ncg = KT > 0 ? (c->g.nzp - 1) / KC : (c->g.nzp + KC - 1) / KC;
+    const int nblocks_main = (int)(((long long)c->g.ncol * ncg + TPB - 1) / TPB);
+    const int nblocks = nblocks_main + (KT > 0 ? (int)((c->g.ncol + TPB - 1) / TPB) : 0);
     const long long nitems = (long long)nblocks * c->plan.adj_nchunk;
     dim3 grid((unsigned)nblocks, c->plan.adj_nchunk);
     if (c->plan.persistent && (EV == 1 || EV == 2) && nitems < (1ll << 31)) {
@@ -164,9 +184,9 @@ static cudaError_t adj_launch(grav_ctx* c, const double* v, double* partial, con
     } else {
         work = nullptr;
     }
-    adjoint_nodes_kernel<TPB, KC, MINB, EV><<<grid, TPB, smem, s>>>(c->g, c->pd, v, partial, ncg,
-                                                                    c->plan.adj_obs_per_chunk, done, work, nblocks,
-                                                                    (int)nitems);
+    adjoint_nodes_kernel<TPB, KC, MINB, EV, KT><<<grid, TPB, smem, s>>>(c->g, c->pd, v, partial, ncg, nblocks_main,
+                                                                        c->plan.adj_obs_per_chunk, done, work, nblocks,
+                                                                        (int)nitems);
     return cudaGetLastError();
 }
 
@@ -186,7 +206,12 @@ cudaError_t launch_adjoint_nodes(grav_ctx* c, const double* v, double* partial, 
             case 4: e = adj_launch<512, 4, 1, 2>(c, v, partial, done, work, s); break;
             case 5: e = adj_launch<384, 5, 1, 2>(c, v, partial, done, work, s); break;
             case 6: e = adj_launch<384, 6, 1, 2>(c, v, partial, done, work, s); break;
-            case 7: e = adj_launch<384, 7, 1, 2>(c, v, partial, done, work, s); break;
+            case 7:
+                if (c->plan.adj_kt == 4) e = adj_launch<384, 7, 1, 2, 4>(c, v, partial, done, work, s);
+                else if (c->plan.adj_kt == 5) e = adj_launch<384, 7, 1, 2, 5>(c, v, partial, done, work, s);
+                else if (c->plan.adj_kt == 6) e = adj_launch<384, 7, 1, 2, 6>(c, v, partial, done, work, s);
+                else e = adj_launch<384, 7, 1, 2>(c, v, partial, done, work, s);
+                break;
             case 11: e = adj_launch<256, 11, 1, 2>(c, v, partial, done, work, s); break;
             case 13: e = adj_launch<256, 13, 1, 2>(c, v, partial, done, work, s); break;
             case 17: e = adj_launch<256, 17, 1, 2>(c, v, partial, done, work, s); break;

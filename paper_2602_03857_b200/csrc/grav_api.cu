@@ -80,8 +80,22 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
         }
         p.adj_tpb = p.adj_kc >= 6 ? 128 : 256;
     }
-    p.adj_ncg = ceil_div(g.nzp, p.adj_kc);
-    p.adj_blocks = ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
+    p.adj_kt = 0;
+    if (log2d) {
+        // whole groups of 7 and ONE tail group of 4-6 nodes instead of a padded last group (adjoint.cu, KT): columns
+        // whose length no compiled KC divides (config 5: 151 nodes) lose up to 6 evaluations per column and station
+        // to the padding otherwise.  The tail group runs at the cost of a short-KC variant.
+        const int nmain = (g.nzp - 1) / 7, rest = g.nzp - nmain * 7;
+        if (nmain >= 1 && rest <= 6) {
+            const int kt = rest < 4 ? 4 : rest;
+            const double tailcyc = kt == 4 ? 118.0 : (kt == 5 ? 116.0 : 115.0);
+            const double cost = 111.5 * 7.0 * nmain + tailcyc * kt;
+            if (cost < best) { best = cost; p.adj_kc = 7; p.adj_tpb = 384; p.adj_kt = kt; }
+        }
+    }
+    p.adj_ncg = p.adj_kt ? (g.nzp - 1) / p.adj_kc + 1 : ceil_div(g.nzp, p.adj_kc);
+    p.adj_blocks = p.adj_kt ? ceil_div((long long)g.ncol * (p.adj_ncg - 1), p.adj_tpb) + ceil_div(g.ncol, p.adj_tpb)
+                            : ceil_div((long long)g.ncol * p.adj_ncg, p.adj_tpb);
     want = ceil_div(log2d ? 148 * 48 : 148 * 128, p.adj_blocks);
     while (want > 1 && (double)want * 2.0 * g.Nn * 8.0 > 256e6) --want;   // [hi|lo] partial planes <= 256 MB
     // a chunk is at least 64 stations (one shared-memory tile is 256); tiny problems, where that leaves fewer blocks

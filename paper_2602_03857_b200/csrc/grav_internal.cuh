@@ -35,6 +35,7 @@ struct Plan {
     int fwd_tpb, fwd_tiles, fwd_nchunk, fwd_cols_per_chunk;
     // adjoint: grid (node-thread blocks, station chunks)
     int adj_tpb, adj_kc, adj_ncg, adj_blocks, adj_nchunk, adj_obs_per_chunk;
+    int adj_kt;            // > 0: the column is covered by whole groups of adj_kc nodes and one tail group of adj_kt (adjoint.cu)
     // per-pair family (stored.cu): node tile of pair_tnx x pair_tny node columns per block
     int pair_tnx, pair_tny, pair_tiles_x, pair_tiles_y;
 };
