@@ -84,11 +84,13 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     if (log2d) {
         // whole groups of 7 and ONE tail group of 4-6 nodes instead of a padded last group (adjoint.cu, KT): columns
         // whose length no compiled KC divides (config 5: 151 nodes) lose up to 6 evaluations per column and station
-        // to the padding otherwise.  The tail group runs at the cost of a short-KC variant.
+        // to the padding otherwise.
         const int nmain = (g.nzp - 1) / 7, rest = g.nzp - nmain * 7;
         if (nmain >= 1 && rest <= 6) {
             const int kt = rest < 4 ? 4 : rest;
-            const double tailcyc = kt == 4 ? 118.0 : (kt == 5 ? 116.0 : 115.0);
+            // measured: 133 cycles per warp-evaluation in the tail group (config 5 with KT = 4: 1853 -> 1826 ms; config 2
+            // with KT = 5 instead of its (256, 11) variant: 1.883 -> 1.910 ms, so config 2 keeps (256, 11))
+            const double tailcyc = 133.0;
             const double cost = 111.5 * 7.0 * nmain + tailcyc * kt;
             if (cost < best) { best = cost; p.adj_kc = 7; p.adj_tpb = 384; p.adj_kt = kt; }
         }
