@@ -443,7 +443,8 @@ def run_ours(args):
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     if int(os.environ.get("WORLD_SIZE", "1")) > 1:
-        os.environ.setdefault("NCCL_DEBUG", "INFO")       # rank / transport lines on stderr (the JSON line is stdout)
+        os.environ.setdefault("NCCL_DEBUG", "INFO")       # rank / transport lines ...
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")   # ... on stderr (NCCL's default is stdout; the JSON line owns stdout)
     # NCCL, one rank per GPU.  GRAV_DIST_BACKEND=gloo (development only): several ranks share the visible GPUs and the
     # collectives are staged through host memory (dist.Comm.staged) - a functional check of this file's multi-rank logic
     # on a one-GPU box, never a measurement.
