@@ -3,8 +3,8 @@
 //   T_n = sum_i v_i Psi(node_n - obs_i);   g_k = gamma * sum_pqr sigma T[corner_pqr(k)]   (nodeops.cu)
 //
 // Transposed tiling: one thread owns KC consecutive nodes of one node column (their z and accumulators live in
-// registers); stations are staged through shared memory in tiles and read at the same address by every thread
-// (broadcast).  X, Y, X*Y, X^2+Y^2 are computed once per (thread, station) and shared by the KC nodes.
+// registers); stations are staged through shared memory, kAdjObsStage per block-wide barrier, and read at the same
+// address by every thread (broadcast).  X, Y, X*Y, X^2+Y^2 are computed once per (thread, station) and shared by the KC nodes.
 // Every node is owned by exactly one thread: no atomics.
 //
 // Accumulation.  T_n is a sum of up to N same-sign terms of size |v Psi| ~ 1e4..1e5 m whose 8-corner signed
@@ -19,7 +19,8 @@
 
 namespace grav {
 
-constexpr int kAdjObsTile = 256;
+constexpr int kAdjObsTile = 256;     // stations per plain running sum (accuracy: 1024 loses 1.1e-10 of max at config 3)
+constexpr int kAdjObsStage = 1024;   // stations staged in shared memory per block-wide barrier
 
 // EV: 0 = CUDA libm (cross-check), 1 = psi_eval with the 256-entry log table, 2 = psi_eval with the 2-D log table,
 // 3 = the Float32 evaluator psi_f32 with FP64 accumulation (grav_set_precision)
@@ -49,43 +50,46 @@ __device__ __forceinline__ void adjoint_item(const Geom& g, const PsiTabView& tb
     const long long i1 = min(i0 + (long long)obs_per_chunk, g.N);
     double* out_hi = partial + (long long)by * 2 * g.Nn + (long long)col * g.nzp + c0;
     double* out_lo = out_hi + g.Nn;
-    for (long long base = i0; base < i1; base += kAdjObsTile) {
-        const int cnt = (int)min((long long)kAdjObsTile, i1 - base);
+    for (long long sbase = i0; sbase < i1; sbase += kAdjObsStage) {
+        const int scnt = (int)min((long long)kAdjObsStage, i1 - sbase);
         __syncthreads();
-        for (int j = threadIdx.x; j < cnt; j += TPB)
-            s_obs[j] = make_double4(g.xo[base + j], g.yo[base + j], g.zo[base + j], v[base + j]);
+        for (int j = threadIdx.x; j < scnt; j += TPB)
+            s_obs[j] = make_double4(g.xo[sbase + j], g.yo[sbase + j], g.zo[sbase + j], v[sbase + j]);
         __syncthreads();
-        for (int j = 0; j < cnt; ++j) {
-            const double4 o = s_obs[j];
-            const double X = xa - o.x, Y = yb - o.y;
-            if (EV == 1 || EV == 2) {
-                const PsiColumn pc = psi_column(X, Y);
-                const double vs = o.w * pc.s;
+        for (int j0 = 0; j0 < scnt; j0 += kAdjObsTile) {
+            const int j1 = min(j0 + kAdjObsTile, scnt);
+            for (int j = j0; j < j1; ++j) {
+                const double4 o = s_obs[j];
+                const double X = xa - o.x, Y = yb - o.y;
+                if (EV == 1 || EV == 2) {
+                    const PsiColumn pc = psi_column(X, Y);
+                    const double vs = o.w * pc.s;
 #pragma unroll
-                for (int k = 0; k < K; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
-            } else if (EV == 3) {
-                const float Xf = (float)X, Yf = (float)Y;
+                    for (int k = 0; k < K; ++k) acc[k] = fma(vs, psi_eval<EV == 2>(tb, pc, zc[k] - o.z), acc[k]);
+                } else if (EV == 3) {
+                    const float Xf = (float)X, Yf = (float)Y;
 #pragma unroll
-                for (int k = 0; k < K; ++k)
-                    acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale, s_at), acc[k]);
-            } else {
-                const double XY = X * Y;
-                const double Q = fma(Y, Y, X * X);
+                    for (int k = 0; k < K; ++k)
+                        acc[k] = fma(o.w, (double)psi_f32(Xf, Yf, (float)(zc[k] - o.z), inv_scale, s_at), acc[k]);
+                } else {
+                    const double XY = X * Y;
+                    const double Q = fma(Y, Y, X * X);
 #pragma unroll
-                for (int k = 0; k < K; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
-            }
-        }
-        // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
-        if (valid) {
-#pragma unroll
-            for (int k = 0; k < K; ++k) {
-                if (c0 + k < g.nzp) {
-                    double hi = acc[k], lo = 0.0;
-                    if (base != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
-                    out_hi[k] = hi;
-                    out_lo[k] = lo;
+                    for (int k = 0; k < K; ++k) acc[k] = fma(o.w, psi_libm(X, Y, zc[k] - o.z, XY, Q), acc[k]);
                 }
-                acc[k] = 0.0;
+            }
+            // fold the tile sum into the (hi, lo) pair of each owned node and restart the running sum
+            if (valid) {
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    if (c0 + k < g.nzp) {
+                        double hi = acc[k], lo = 0.0;
+                        if (sbase + j0 != i0) two_sum_acc(out_hi[k], out_lo[k], acc[k], hi, lo);
+                        out_hi[k] = hi;
+                        out_lo[k] = lo;
+                    }
+                    acc[k] = 0.0;
+                }
             }
         }
     }
@@ -105,7 +109,7 @@ __global__ void __launch_bounds__(TPB, MINB) adjoint_nodes_kernel(Geom g, PsiDev
                                                                   int* __restrict__ work, int nblocks, int nitems) {
     extern __shared__ double2 s_tab[];
     if (done && *done) return;
-    __shared__ double4 s_obs[kAdjObsTile];   // (xo, yo, zo, v)
+    __shared__ double4 s_obs[kAdjObsStage];   // (xo, yo, zo, v)
     __shared__ int s_item;
     __shared__ float s_at[kAtanN32];
     PsiTabView tb;
