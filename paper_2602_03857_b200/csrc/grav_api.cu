@@ -56,6 +56,23 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     while (want > 1 && (double)want * g.N * 8.0 > 64e6) --want;      // partial buffer <= 64 MB
     if (want < 1) want = 1;
     p.fwd_cols_per_chunk = ceil_div(g.ncol, want);
+    if (log2d) {
+        // One block per SM is resident, every block of a launch takes the same time (cols_per_chunk columns), so the
+        // launch costs ceil(blocks / SMs) rounds: among the chunk sizes between `want` chunks and ~8 rounds pick the one
+        // with the cheapest rounds x (columns per chunk + per-block overhead).  The overhead - drawing the item, the
+        // first copy of node data, the barriers - is ~3 us (persistent launch) or ~1 us, in units of one column's time
+        // (config 2: 1.820 -> 1.76 ms; the sweep of chunk counts there is not monotonic: 1.76 to 1.83 ms).
+        const double t_col = (double)g.nzp * 4.0 * 109.4 / 1.965e9;
+        const double ovh = (p.persistent ? 3e-6 : 1e-6) / t_col;
+        const int cols_lo = p.fwd_cols_per_chunk;
+        const int cols_hi = std::max(cols_lo, ceil_div((long long)g.ncol * p.fwd_tiles, (long long)sms * 8));
+        double best_cost = 1e300;
+        for (int cols = cols_lo; cols <= cols_hi; ++cols) {
+            const long long blocks = (long long)ceil_div(g.ncol, cols) * p.fwd_tiles;
+            const double cost = (double)ceil_div(blocks, sms) * ((double)cols + ovh);
+            if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; p.fwd_cols_per_chunk = cols; }
+        }
+    }
     p.fwd_nchunk = ceil_div(g.ncol, p.fwd_cols_per_chunk);
     p.fwd_reduce_rx = g.N < 32 * kDotBlocks ? 8 : 32;      // few stations: 8 per block and 32 chunk lanes (forward.cu)
     // adjoint: one thread per (node column, group of KC layers); split the stations into chunks when few threads
@@ -109,6 +126,20 @@ void make_plan(const Geom& g, const PsiDev& pd, bool log2d, int sms, Plan& p) {
     if (want > 256) want = 256;
     if (want < 1) want = 1;
     p.adj_obs_per_chunk = ceil_div(g.N, want);
+    if (log2d) {
+        // the same fit of rounds to the SM count as for the forward chunks: among 1..want station chunks (at least ~8
+        // rounds) the cheapest rounds x (stations per chunk + per-block overhead in stations' time)
+        const double t_obs = (double)p.adj_kc * 111.5 * (p.adj_tpb / 128) / 1.965e9;
+        const double ovh = (p.persistent ? 3e-6 : 1e-6) / t_obs;
+        double best_cost = 1e300;
+        for (int nch = want; nch >= 1; --nch) {
+            const int obs = ceil_div(g.N, nch);
+            const long long blocks = (long long)ceil_div(g.N, obs) * p.adj_blocks;
+            if (nch < want && blocks < (long long)sms * 8) break;
+            const double cost = (double)ceil_div(blocks, sms) * ((double)obs + ovh);
+            if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; p.adj_obs_per_chunk = obs; }
+        }
+    }
     p.adj_nchunk = ceil_div(g.N, p.adj_obs_per_chunk);
     make_pair_plan(g, pd, log2d, p);
 }
